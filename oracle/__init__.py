@@ -1,0 +1,23 @@
+"""fp64 CPU oracle for the deltaMic mesh Fourier transform -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It shares no code with paper_2303_10440_b200 (the CUDA path) and neither imports the
+other.  See oracle/mesh_ft_oracle.c for the definitions and citations, oracle/render.py for the
+image-formation reference (PSF multiply + inverse rFFT).
+
+Parity status: every function here is pinned by `-m "not gpu"` tests (tests/test_oracle_*.py) except
+the behaviour of an inverse real FFT on a half spectrum that is not exactly Hermitian on its
+self-conjugate planes (reading R13), where the oracle *defines* the semantics as numpy/pocketfft's
+irfftn -- "parity unpinned" for that one convention.
+"""
+from .mesh_ft import (  # noqa: F401
+    frequency_grid,
+    g_fun,
+    g_grad,
+    mesh_ft_forward,
+    mesh_ft_forward_grid,
+    mesh_ft_backward,
+    mesh_ft_backward_grid,
+    num_threads,
+)
+from .render import psf_shift_spectrum, render, render_backward, spectrum_to_image, image_to_spectrum_cotangent  # noqa: F401
