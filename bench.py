@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py -- mesh-FT throughput of the B200-native deltaMic hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--cfg C] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one synthetic workload: dm_mesh_ft_forward (rows A1-A5) then
+dm_mesh_ft_backward (rows A1, A6, A7) with a spectrum cotangent resident in HBM.  The metric is (triangle x
+frequency) pairs per second over forward+backward; the forward-only / backward-only rates and the "ms per render
+at 128^3" (dm_render of the same workload, with its stage split) ride along in the same JSON line.
+
+Default workload at N=1: config 4 of BASELINE.json (surface mode, 20 membranes, 102 400 triangles, 128^3 grid), the
+configuration the north_star target is quoted on.  N>1 (torchrun): every rank processes its own mesh of the same
+recipe (seed + rank) -- independent problems, no data-path collective, weak scaling; value = all ranks' pairs / max time.
+
+--impl reference times the fp64 CPU oracle (oracle/, as it stands) on a bounded frequency sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "mesh-FT (triangle*frequency) pairs/s fwd+bwd"
+UNIT = "pairs/s"
+# SURVEY.md section 8(d) / DESIGN.md section 7: algorithmic FP32 lane-ops per (triangle, frequency) pair
+FLOOR_OPS = {"fwd": {0: 26.0, 1: 23.0}, "bwd": {0: 60.0, 1: 60.0}}
+FP32_LANES_PER_CLK_PER_SM = 128
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d.get("sm_max_mhz", 1965.0)), "MEASURED_PEAKS.json sm_max_mhz"
+    return 1965.0, "fallback clocks.max.sm 1965 MHz (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self._stop = threading.Event()
+        self._thr = None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.QUERY}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [p.strip() for p in out.strip().split(",")]
+                if len(parts) >= 7:
+                    self.rows.append(parts)
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._thr.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
+                "samples": len(self.rows), "power_w_max": max(float(r[2]) for r in self.rows)}
+
+
+def oracle_sample(w, n_freq: int, seed: int = 0):
+    """Times the oracle (forward + backward) on ``n_freq`` random stored frequencies of workload ``w``."""
+    import oracle
+    from workloads.configs import spectrum_cotangent
+
+    rng = np.random.default_rng(seed)
+    idx = np.sort(rng.choice(w.n_k, size=min(n_freq, w.n_k), replace=False))
+    G = spectrum_cotangent(w).reshape(-1)[idx].astype(np.complex128)
+    t0 = time.perf_counter()
+    oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, w.mode, flat_indices=idx)
+    t1 = time.perf_counter()
+    oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, w.mode, G, flat_indices=idx)
+    t2 = time.perf_counter()
+    pairs = float(w.faces.shape[0]) * len(idx)
+    return {"pairs": pairs, "fwd_s": t1 - t0, "bwd_s": t2 - t1, "n_freq": int(len(idx)), "cores": oracle.num_threads()}
+
+
+def run_reference(args):
+    """The reference arm of this tier = the oracle, timed on host cores on a bounded sample of the workload."""
+    from workloads import build_workload
+
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = build_workload(args.cfg)
+    n_freq = max(8, int(args.ref_freqs))
+    for _ in range(max(0, args.warmup)):
+        oracle_sample(w, max(4, n_freq // 8))
+    res = [oracle_sample(w, n_freq, seed=s) for s in range(max(1, args.steps))]
+    t = sum(r["fwd_s"] + r["bwd_s"] for r in res) / len(res)
+    value = res[0]["pairs"] / t
+    sample = f"{res[0]['n_freq']} random stored frequencies x all {w.faces.shape[0]} triangles per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "cfg": args.cfg, "mode": "surface" if w.mode else "volume",
+                   "n_triangles": int(w.faces.shape[0]), "grid": list(w.n), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": res[0]["cores"], "kind": "oracle", "sample": sample,
+                         "fwd_pairs_s": res[0]["pairs"] / np.mean([r["fwd_s"] for r in res]),
+                         "bwd_pairs_s": res[0]["pairs"] / np.mean([r["bwd_s"] for r in res])},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2303_10440_b200 as dm
+    from workloads import build_workload
+    from workloads.configs import image_cotangent, spectrum_cotangent
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dm.load_library()  # fails loudly when the CUDA extension is missing
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # every rank owns one mesh of the same recipe (independent problems; seed offset = rank)
+    w = build_workload(args.cfg, seed_offset=rank)
+    plan = dm.Plan(w.n, w.spacing, w.origin, w.mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    vd = torch.as_tensor(w.vertices, device="cuda")
+    Gd = torch.as_tensor(spectrum_cotangent(w), device="cuda")
+    F = torch.empty(w.spectrum_shape, dtype=torch.complex64, device="cuda")
+    dv = torch.empty((w.vertices.shape[0], 3), dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(ev):
+        flush.fill_(1)  # L2 flush between timed iterations (outside the events)
+        ev[0].record(stream)
+        plan.mesh_ft_forward(vd, out=F)
+        ev[1].record(stream)
+        plan.mesh_ft_backward(vd, Gd, out=dv)
+        ev[2].record(stream)
+
+    def new_ev():
+        return [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+
+    for _ in range(max(args.warmup, 0)):
+        step(new_ev())
+    launches0 = plan.launch_count()
+    barrier()
+    evs = [new_ev() for _ in range(args.steps)]
+    bwd_kernel_ms = []
+    with ClockSampler(local) as clk:
+        t_wall0 = time.perf_counter()
+        for ev in evs:
+            step(ev)
+            bwd_kernel_ms.append(plan.stage_ms()["mesh_ft"])  # syncs; = A1 + A6 kernel time of this step's backward
+        barrier()
+        t_wall = time.perf_counter() - t_wall0
+    launches = plan.launch_count() - launches0
+    fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    bwd_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    step_ms = fwd_ms + bwd_ms
+    t = torch.tensor([step_ms, fwd_ms, bwd_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    step_ms, fwd_ms, bwd_ms = (float(x) for x in t.tolist())
+    pairs = float(w.pairs)
+
+    # ---- end to end through the public API with HOST buffers (render + render_backward) ---------------------------
+    hv = torch.as_tensor(w.vertices).pin_memory()
+    hg = torch.as_tensor(image_cotangent(w) if w.cfg in (1, 3, 5) else
+                         np.random.default_rng(10 + w.seed).standard_normal(w.n).astype(np.float32)).pin_memory()
+    himg = torch.empty(w.n, dtype=torch.float32).pin_memory()
+    hdv = torch.empty((w.vertices.shape[0], 3), dtype=torch.float32).pin_memory()
+    gimg = torch.empty(w.n, dtype=torch.float32, device="cuda")
+    ggrad = torch.empty(w.n, dtype=torch.float32, device="cuda")
+    render_ms, stage = [], {}
+
+    def e2e_step():
+        vd.copy_(hv, non_blocking=True)
+        ggrad.copy_(hg, non_blocking=True)
+        plan.render(vd, w.psf_cov, out=gimg)
+        himg.copy_(gimg, non_blocking=True)
+        plan.render_backward(vd, w.psf_cov, ggrad, out=dv)
+        hdv.copy_(dv, non_blocking=True)
+
+    e2e_step()
+    barrier()
+    e2e_n = max(1, min(args.steps, 3))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(e2e_n):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    e2e_ms = e0.elapsed_time(e1) / e2e_n
+    t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item())
+    # ms per render (forward only) with its stage split
+    for _ in range(3):
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record(stream)
+        plan.render(vd, w.psf_cov, out=gimg)
+        r1.record(stream)
+        stage = plan.stage_ms()
+        render_ms.append(r0.elapsed_time(r1))
+    h2d = hv.numel() * 4 + hg.numel() * 4
+    d2h = himg.numel() * 4 + hdv.numel() * 4
+
+    if rank == 0:
+        sm_max_mhz, peak_src = _peaks()
+        n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+        clocks = clk.summary()
+        peak = FP32_LANES_PER_CLK_PER_SM * n_sm * sm_max_mhz * 1e6 / 1e12  # T lane-op/s
+        bk_ms = float(np.mean(bwd_kernel_ms))
+        achieved = FLOOR_OPS["bwd"][w.mode] * pairs / (bk_ms * 1e-3) / 1e12
+        sm_mhz = clocks.get("sm_mhz") or sm_max_mhz
+        roofline = {
+            "bound": "alu", "kernel": "dm_k_backward (A6, dominant)", "achieved": achieved, "peak": peak,
+            "unit": "T lane-op/s (FP32 issue: 128 lanes/clk/SM)", "frac": achieved / peak, "traffic": None,
+            "peak_source": f"128 x {n_sm} SMs x {sm_max_mhz:.0f} MHz ({peak_src}); DESIGN.md section 7",
+            "frac_at_measured_clock": achieved / (peak * sm_mhz / sm_max_mhz),
+            "algorithmic_ops_per_pair": FLOOR_OPS["bwd"][w.mode], "kernel_ms": bk_ms,
+            "forward": {"achieved": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12,
+                        "frac": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12 / peak,
+                        "algorithmic_ops_per_pair": FLOOR_OPS["fwd"][w.mode]},
+        }
+        o = oracle_sample(w, args.ref_freqs)
+        sample = f"{o['n_freq']} random stored frequencies x all {w.faces.shape[0]} triangles, forward+backward"
+        line = {
+            "metric": METRIC, "value": world * pairs / (step_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "cfg": w.cfg, "mode": "surface" if w.mode else "volume",
+                       "n_triangles": int(w.faces.shape[0]), "n_vertices": int(w.vertices.shape[0]), "grid": list(w.n),
+                       "pairs_per_pass": pairs, "l2": "flushed between timed iterations (256 MB write)",
+                       "parallelism": f"replicas x{world}"},
+            "fwd_pairs_s": world * pairs / (fwd_ms * 1e-3), "bwd_pairs_s": world * pairs / (bwd_ms * 1e-3),
+            "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
+            "render_ms": float(np.median(render_ms)), "render_stage_ms": stage,
+            "e2e": {"value": world * pairs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
+                    "what": "dm_render + dm_render_backward with pinned host vertices/dL_dimage in, image/dL_dv out"},
+            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
+            "cpu_baseline": {"value": o["pairs"] / (o["fwd_s"] + o["bwd_s"]), "unit": UNIT, "cores": o["cores"],
+                             "kind": "oracle", "sample": sample, "fwd_pairs_s": o["pairs"] / o["fwd_s"],
+                             "bwd_pairs_s": o["pairs"] / o["bwd_s"]},
+            "wall_s_timed_region": t_wall,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json config 1..5 (default 4, the target config)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-freqs", type=int, default=192, help="stored frequencies per oracle sample")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

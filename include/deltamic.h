@@ -1,0 +1,139 @@
+/*
+ * deltamic.h -- C ABI of the B200-native (sm_100a) mesh Fourier transform of deltaMic
+ * (arxiv 2303.10440, "Differentiable Rendering for 3D Fluorescence Microscopy").
+ *
+ * Citations are "PAPER.md:<line>" of the paper text plus the equation they fall in; "north_star" is
+ * BASELINE.json's statement of the build.  Readings R1..R24 are listed in DESIGN.md section 3.
+ *
+ * The library renders a triangle mesh into a 3D image through the Fourier domain (Fig. 1,
+ * :83-89 eq. 1-2):   image = irfft3( F . h_hat . e^{+i k.x0} ) / (h_x h_y h_z),
+ * where F is the continuous Fourier transform of the mesh sampled on the image's rfft half-spectrum grid
+ * (the hot path: dm_mesh_ft_forward / dm_mesh_ft_backward) and h_hat the spectrum of a Gaussian PSF
+ * (eq. 3-4, reading R5).  Every step runs in CUDA kernels on one GPU; there is no CPU
+ * fallback and no other backend.
+ *
+ * Conventions
+ *  - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. torch tensors' data_ptr());
+ *    pointers named *_host are host pointers.  The plan owns its workspace and frees it in dm_plan_destroy.
+ *  - Frequency grid (reading R10): spectrum arrays are [n_x][n_y][n_z/2+1], z fastest, complex64
+ *    interleaved (re, im).  Index (i_x,i_y,i_z) holds integer frequency n_a = i_a for i_a < N_a/2,
+ *    i_a - N_a otherwise (numpy fftfreq order) on x and y, n_z = i_z = 0..N_z/2; the angular frequency
+ *    is k_a = 2 pi n_a / (N_a * spacing_a)  (PAPER.md:131 uses the angular convention e^{-i z.xi}).
+ *  - Image arrays are [n_x][n_y][n_z] float32, z fastest.  Voxel (i,j,l) samples the point
+ *    origin + (i h_x, j h_y, l h_z)  (readings R9, R11).
+ *  - Vertices are float32 [n_vertices][3]; faces int32 [n_faces][3], counter-clockwise seen from outside
+ *    (outward normal) -- a documented precondition of DM_VOLUME, not checked (reading R8).
+ *  - Calls are asynchronous on the plan's CUDA stream unless stated.  Every call returns DM_OK (0) or a
+ *    negative dm_status; nothing aborts, throws or prints.  Launch errors are returned by the call that
+ *    made them, execution errors by the next call or the caller's own synchronisation.
+ */
+#ifndef DELTAMIC_H
+#define DELTAMIC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dm_plan dm_plan; /* opaque */
+
+typedef struct dm_grid {
+    int32_t n[3];       /* voxels (x, y, z); the rfft half axis is z; n[2] must be even        */
+    float   spacing[3]; /* voxel size per axis; box length L_a = n[a] * spacing[a]             */
+    float   origin[3];  /* sample point of voxel (0,0,0) (its centre), reading R11             */
+} dm_grid;
+
+typedef enum dm_mode {
+    DM_VOLUME  = 0, /* F(k) = int_Omega e^{-ik.x} d^3x  (indicator of the enclosed volume; north_star)   */
+    DM_SURFACE = 1  /* F(k) = sum_T int_T e^{-ik.x} dS  (membrane density; eq. 8-9,
+                       :177-180 eq. 12 without the 1/|Lambda| normalisation, reading R7)                 */
+} dm_mode;
+
+typedef enum dm_status {
+    DM_OK              =  0,
+    DM_ERR_INVALID_ARG = -1, /* null pointer, non-positive size, odd n_z, unknown mode, bad slab        */
+    DM_ERR_BAD_MESH    = -2, /* a face index is outside [0, n_vertices)                                 */
+    DM_ERR_ALLOC       = -3, /* host or device allocation failed                                        */
+    DM_ERR_CUDA        = -4, /* a CUDA runtime call or kernel launch failed                             */
+    DM_ERR_CUFFT       = -5, /* a cuFFT call failed                                                     */
+    DM_ERR_UNSUPPORTED = -6  /* the requested feature is not built                                      */
+} dm_status;
+
+/* Create a plan for one grid, mode and mesh topology.
+ *   faces_dev  device int32 [n_faces*3]; read (and validated) here and copied: the caller may free it
+ *              afterwards.  A topology change needs a new plan; vertex positions may change freely.
+ *   cuda_stream  a cudaStream_t (as void*); NULL = the legacy default stream.  All later calls on the
+ *              plan are ordered on it.
+ * This call synchronises the stream (it builds the vertex->corner CSR map of PAPER.md:182-186 eq. 13
+ * and the cuFFT plans).  Returns DM_ERR_BAD_MESH for an out-of-range face index. */
+int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_vertices, int32_t n_faces,
+                   const int32_t* faces_dev, void* cuda_stream);
+
+/* Restrict the mesh-FT calls of this plan to the x-slab [ix_begin, ix_end) of the stored spectrum
+ * (array rows, not signed frequencies).  dm_mesh_ft_forward then writes only those rows of F and
+ * dm_mesh_ft_backward sums only over them (a partial dL/dv that the caller all-reduces over slabs;
+ * DESIGN.md section 9).  Default: the whole grid.  dm_render* require the whole grid. */
+int dm_plan_set_slab(dm_plan* plan, int32_t ix_begin, int32_t ix_end);
+
+/* Mesh Fourier transform (the hot path, forward).
+ *   surface: F(k) = sum_T 2 A_T f_T(k),  f_T = eq. 9, evaluated through a numerically
+ *            stable branch (series / divided differences) where the denominators of eq. 9 vanish or nearly
+ *            vanish (eq. 14-16 done to full order, reading R4);
+ *   volume:  F(k) = (i/|k|^2) sum_T (k.m_T) f_T(k),  m_T = (v2-v1)x(v3-v1),  F(0) = 1/6 sum_T v1.(v2 x v3).
+ *   vertices_dev  float32 [n_vertices*3]
+ *   F_dev         complex64 [n_x*n_y*(n_z/2+1)], overwritten (only the slab rows if a slab is set). */
+int dm_mesh_ft_forward(dm_plan* plan, const float* vertices_dev, float* F_dev);
+
+/* Vertex gradient of the mesh FT (the hot path, backward; PAPER.md:165-173 eq. 10-11, :182-186 eq. 13).
+ *   dL_dF_dev  complex64, layout of F: G = dL/dRe F + i dL/dIm F for every STORED entry, all entries
+ *              independent (reading R14).
+ *   dL_dvertices_dev  float32 [n_vertices*3], overwritten with  sum_k Re( conj(G(k)) dF(k)/dv ).
+ * Reduction over k per triangle is atomic-free and the scatter to vertices is a gather through the CSR
+ * vertex->corner map, so results are bitwise reproducible run to run. */
+int dm_mesh_ft_backward(dm_plan* plan, const float* vertices_dev, const float* dL_dF_dev,
+                        float* dL_dvertices_dev);
+
+/* Whole forward render: mesh FT, multiply by the PSF spectrum and the origin shift, inverse real FFT.
+ *   psf_cov_host  6 floats on the HOST: covariance of the Gaussian PSF in physical units, order
+ *                 xx, yy, zz, xy, xz, yz;  h_hat(k) = exp(-1/2 k^T Sigma k)  (eq. 4 with reading R5).
+ *   image_dev     float32 [n_x*n_y*n_z], overwritten. */
+int dm_render(dm_plan* plan, const float* vertices_dev, const float* psf_cov_host, float* image_dev);
+
+/* Backward of dm_render with respect to the vertices.
+ *   dL_dimage_dev      float32 [n_x*n_y*n_z]
+ *   dL_dvertices_dev   float32 [n_vertices*3], overwritten
+ *   dL_dpsf_cov_host   NULL, or 6 floats on the host; a non-NULL pointer returns DM_ERR_UNSUPPORTED
+ *                      until the PSF-parameter gradient is built. */
+int dm_render_backward(dm_plan* plan, const float* vertices_dev, const float* psf_cov_host,
+                       const float* dL_dimage_dev, float* dL_dvertices_dev, float* dL_dpsf_cov_host);
+
+/* The two surrounding stages on their own (used by the tests and the stage timing):
+ *   dm_spectrum_to_image:  image = irfft3( F . h_hat . e^{+ik.x0} ) / (h_x h_y h_z)
+ *   dm_image_to_spectrum_cotangent:  G = conj(h_hat e^{+ik.x0}) . w . rfft3(dL/dimage) / (N_tot h_x h_y h_z),
+ *       w = 1 on the planes n_z = 0 and n_z = N_z/2, else 2 (the adjoint of the half-spectrum inverse
+ *       transform on independent stored entries, reading R14).
+ * F_dev is not modified. */
+int dm_spectrum_to_image(dm_plan* plan, const float* F_dev, const float* psf_cov_host, float* image_dev);
+int dm_image_to_spectrum_cotangent(dm_plan* plan, const float* dL_dimage_dev, const float* psf_cov_host,
+                                   float* G_dev);
+
+/* Device time of the stages of the LAST dm_render / dm_render_backward / dm_mesh_ft_* call, in ms:
+ * ms[0] mesh FT (forward or backward reduction), ms[1] PSF multiply, ms[2] FFT, ms[3] scatter to
+ * vertices.  Stages a call did not run report 0.  Synchronises the plan's stream. */
+int dm_plan_stage_ms(dm_plan* plan, float ms[4]);
+
+/* Number of CUDA kernels (cuFFT's excluded) the plan has launched since creation. */
+int64_t dm_plan_launch_count(const dm_plan* plan);
+
+void dm_plan_destroy(dm_plan* plan);
+
+const char* dm_error_string(int code);
+
+/* Library version as major*10000 + minor*100 + patch. */
+int dm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DELTAMIC_H */

@@ -1,0 +1,20 @@
+"""paper_2303_10440_b200 -- B200-native (sm_100a) mesh Fourier transform of deltaMic (arxiv 2303.10440).
+
+Thin ctypes binding over the C-ABI library ``libdeltamic.so`` (declared in ``include/deltamic.h``): argument
+marshalling only, every step of the path runs in the library's CUDA kernels.  PyTorch supplies device memory and
+streams.  There is no CPU fallback: importing the binding without the built library, or calling it without a CUDA
+device, raises.
+"""
+from ._binding import (  # noqa: F401
+    DM_SURFACE,
+    DM_VOLUME,
+    DeltamicError,
+    Plan,
+    exported_symbols,
+    library_path,
+    load_library,
+    version,
+)
+
+__all__ = ["Plan", "DM_VOLUME", "DM_SURFACE", "DeltamicError", "load_library", "library_path", "exported_symbols",
+           "version"]

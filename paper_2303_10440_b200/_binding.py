@@ -1,0 +1,230 @@
+"""ctypes binding of include/deltamic.h.  Same names as the C ABI, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(HERE, "libdeltamic.so")
+
+DM_VOLUME, DM_SURFACE = 0, 1
+
+# every symbol include/deltamic.h declares
+_SYMBOLS = (
+    "dm_plan_create", "dm_plan_set_slab", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_render",
+    "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
+    "dm_plan_launch_count", "dm_plan_destroy", "dm_error_string", "dm_version",
+)
+
+
+class DeltamicError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what} failed: {code} ({_err(code)})")
+        self.code = code
+
+
+class _Grid(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int32 * 3), ("spacing", ctypes.c_float * 3), ("origin", ctypes.c_float * 3)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def exported_symbols():
+    return _SYMBOLS
+
+
+def load_library():
+    """dlopen libdeltamic.so.  Raises (never falls back) when the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_2303_10440_b200.build` "
+            "(there is no CPU fallback)")
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, fp, ip = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p
+    lib.dm_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(_Grid), ctypes.c_int, ctypes.c_int32,
+                                   ctypes.c_int32, ip, vp]
+    lib.dm_plan_set_slab.argtypes = [vp, ctypes.c_int32, ctypes.c_int32]
+    lib.dm_mesh_ft_forward.argtypes = [vp, fp, fp]
+    lib.dm_mesh_ft_backward.argtypes = [vp, fp, fp, fp]
+    lib.dm_render.argtypes = [vp, fp, ctypes.POINTER(ctypes.c_float), fp]
+    lib.dm_render_backward.argtypes = [vp, fp, ctypes.POINTER(ctypes.c_float), fp, fp, ctypes.POINTER(ctypes.c_float)]
+    lib.dm_spectrum_to_image.argtypes = [vp, fp, ctypes.POINTER(ctypes.c_float), fp]
+    lib.dm_image_to_spectrum_cotangent.argtypes = [vp, fp, ctypes.POINTER(ctypes.c_float), fp]
+    lib.dm_plan_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    lib.dm_plan_launch_count.argtypes = [vp]
+    lib.dm_plan_launch_count.restype = ctypes.c_int64
+    lib.dm_plan_destroy.argtypes = [vp]
+    lib.dm_plan_destroy.restype = None
+    lib.dm_error_string.argtypes = [ctypes.c_int]
+    lib.dm_error_string.restype = ctypes.c_char_p
+    lib.dm_version.restype = ctypes.c_int
+    for name in _SYMBOLS:
+        fn = getattr(lib, name)
+        if name not in ("dm_plan_launch_count", "dm_plan_destroy", "dm_error_string"):
+            fn.restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _err(code: int) -> str:
+    try:
+        return load_library().dm_error_string(int(code)).decode()
+    except Exception:  # pragma: no cover
+        return "?"
+
+
+def version() -> int:
+    return int(load_library().dm_version())
+
+
+def _check(code: int, what: str):
+    if code != 0:
+        raise DeltamicError(code, what)
+
+
+def _cov(psf_cov):
+    vals = [float(x) for x in psf_cov]
+    if len(vals) != 6:
+        raise ValueError("psf_cov must hold 6 numbers: xx, yy, zz, xy, xz, yz")
+    return (ctypes.c_float * 6)(*vals)
+
+
+class Plan:
+    """One grid + mode + mesh topology (dm_plan).  Tensors are torch CUDA tensors; all work is queued on
+    ``torch.cuda.current_stream()`` at construction time."""
+
+    def __init__(self, n, spacing, origin, mode: int, faces, n_vertices: int, stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2303_10440_b200 needs a CUDA device (no CPU fallback)")
+        lib = load_library()
+        self._torch = torch
+        self.n = tuple(int(v) for v in n)
+        self.mode = int(mode)
+        self.n_vertices = int(n_vertices)
+        faces = faces if isinstance(faces, torch.Tensor) else torch.as_tensor(faces)
+        faces = faces.to(device="cuda", dtype=torch.int32).contiguous()
+        self.n_faces = int(faces.shape[0])
+        self.device = faces.device
+        self.stream = torch.cuda.current_stream(self.device) if stream is None else stream
+        g = _Grid()
+        for d in range(3):
+            g.n[d] = self.n[d]
+            g.spacing[d] = float(spacing[d])
+            g.origin[d] = float(origin[d])
+        h = ctypes.c_void_p()
+        _check(lib.dm_plan_create(ctypes.byref(h), ctypes.byref(g), self.mode, self.n_vertices, self.n_faces,
+                                  faces.data_ptr(), self.stream.cuda_stream), "dm_plan_create")
+        self._h = h
+        self._lib = lib
+
+    # -- helpers ---------------------------------------------------------------------------------------------
+    @property
+    def spectrum_shape(self):
+        return (self.n[0], self.n[1], self.n[2] // 2 + 1)
+
+    def _f32(self, t, numel, name):
+        torch = self._torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+            raise ValueError(f"{name} must be a contiguous CUDA tensor")
+        if t.dtype == torch.complex64:
+            t = torch.view_as_real(t)
+        if t.dtype != torch.float32 or t.numel() != numel:
+            raise ValueError(f"{name}: expected {numel} float32 values, got {t.numel()} of {t.dtype}")
+        return t
+
+    def _vertices(self, v):
+        return self._f32(v, self.n_vertices * 3, "vertices")
+
+    def _nk(self):
+        return self.n[0] * self.n[1] * (self.n[2] // 2 + 1)
+
+    # -- the C ABI, one method per entry point ------------------------------------------------------------------
+    def set_slab(self, ix_begin: int, ix_end: int):
+        _check(self._lib.dm_plan_set_slab(self._h, int(ix_begin), int(ix_end)), "dm_plan_set_slab")
+
+    def mesh_ft_forward(self, vertices, out=None):
+        torch = self._torch
+        v = self._vertices(vertices)
+        if out is None:
+            out = torch.zeros(self.spectrum_shape, dtype=torch.complex64, device=self.device)
+        o = self._f32(out, 2 * self._nk(), "F")
+        _check(self._lib.dm_mesh_ft_forward(self._h, v.data_ptr(), o.data_ptr()), "dm_mesh_ft_forward")
+        return out
+
+    def mesh_ft_backward(self, vertices, dL_dF, out=None):
+        torch = self._torch
+        v = self._vertices(vertices)
+        g = self._f32(dL_dF, 2 * self._nk(), "dL_dF")
+        if out is None:
+            out = torch.empty((self.n_vertices, 3), dtype=torch.float32, device=self.device)
+        o = self._f32(out, self.n_vertices * 3, "dL_dvertices")
+        _check(self._lib.dm_mesh_ft_backward(self._h, v.data_ptr(), g.data_ptr(), o.data_ptr()), "dm_mesh_ft_backward")
+        return out
+
+    def render(self, vertices, psf_cov, out=None):
+        torch = self._torch
+        v = self._vertices(vertices)
+        if out is None:
+            out = torch.empty(self.n, dtype=torch.float32, device=self.device)
+        o = self._f32(out, self.n[0] * self.n[1] * self.n[2], "image")
+        _check(self._lib.dm_render(self._h, v.data_ptr(), _cov(psf_cov), o.data_ptr()), "dm_render")
+        return out
+
+    def render_backward(self, vertices, psf_cov, dL_dimage, out=None):
+        torch = self._torch
+        v = self._vertices(vertices)
+        g = self._f32(dL_dimage, self.n[0] * self.n[1] * self.n[2], "dL_dimage")
+        if out is None:
+            out = torch.empty((self.n_vertices, 3), dtype=torch.float32, device=self.device)
+        o = self._f32(out, self.n_vertices * 3, "dL_dvertices")
+        _check(self._lib.dm_render_backward(self._h, v.data_ptr(), _cov(psf_cov), g.data_ptr(), o.data_ptr(), None),
+               "dm_render_backward")
+        return out
+
+    def spectrum_to_image(self, F, psf_cov, out=None):
+        torch = self._torch
+        f = self._f32(F, 2 * self._nk(), "F")
+        if out is None:
+            out = torch.empty(self.n, dtype=torch.float32, device=self.device)
+        o = self._f32(out, self.n[0] * self.n[1] * self.n[2], "image")
+        _check(self._lib.dm_spectrum_to_image(self._h, f.data_ptr(), _cov(psf_cov), o.data_ptr()), "dm_spectrum_to_image")
+        return out
+
+    def image_to_spectrum_cotangent(self, dL_dimage, psf_cov, out=None):
+        torch = self._torch
+        g = self._f32(dL_dimage, self.n[0] * self.n[1] * self.n[2], "dL_dimage")
+        if out is None:
+            out = torch.empty(self.spectrum_shape, dtype=torch.complex64, device=self.device)
+        o = self._f32(out, 2 * self._nk(), "G")
+        _check(self._lib.dm_image_to_spectrum_cotangent(self._h, g.data_ptr(), _cov(psf_cov), o.data_ptr()),
+               "dm_image_to_spectrum_cotangent")
+        return out
+
+    def stage_ms(self):
+        ms = (ctypes.c_float * 4)()
+        _check(self._lib.dm_plan_stage_ms(self._h, ms), "dm_plan_stage_ms")
+        return {"mesh_ft": ms[0], "psf": ms[1], "fft": ms[2], "scatter": ms[3]}
+
+    def launch_count(self) -> int:
+        return int(self._lib.dm_plan_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.dm_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,424 @@
+// deltamic.cu -- plan object and C ABI (include/deltamic.h) of the B200-native deltaMic mesh Fourier transform.
+// Host logic only; the arithmetic lives in dm_math.cuh / dm_kernels.cuh / dm_fast.cuh.
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/deltamic.h"
+#include "dm_kernels.cuh"
+
+#define DM_VERSION 100
+
+struct dm_plan {
+    dm_grid grid;
+    DmGridDev gd;
+    int mode;
+    int32_t n_vertices, n_faces;
+    int ix_begin, ix_end;
+    cudaStream_t stream;
+    int n_sm;
+    // device workspace
+    int32_t* faces = nullptr;        // [n_faces*3]
+    int32_t* csr_off = nullptr;      // [n_vertices+1]
+    int32_t* csr_corner = nullptr;   // [n_faces*3]   3*face+corner, ascending per vertex
+    float4* rec = nullptr;           // [n_faces*4]   triangle records (A1)
+    float* part = nullptr;           // [n_split_max*13*n_faces]
+    float* corner = nullptr;         // [n_faces*9]
+    float2* spec = nullptr;          // [n_k] scratch spectrum (S, R or G)
+    float2* spec2 = nullptr;         // [n_k] F or G inside dm_render*
+    int n_split_max = 0;
+    cufftHandle fft_xy = 0, fft_z = 0, fft_r2c = 0;
+    bool have_xy = false, have_z = false, have_r2c = false, have_fft = false;
+    // stage timing
+    cudaEvent_t ev[8];
+    bool ev_ok = false;
+    bool stage_ran[4] = {false, false, false, false};
+    int64_t launches = 0;
+};
+
+namespace {
+
+const char* kErr[] = {"ok", "invalid argument", "bad mesh (face index out of range)", "allocation failed",
+                      "CUDA error", "cuFFT error", "unsupported"};
+
+inline size_t n_k_of(const dm_plan* p) { return (size_t)p->gd.nx * p->gd.ny * p->gd.nzh; }
+
+#define DM_CUDA(x)                            \
+    do {                                      \
+        if ((x) != cudaSuccess) return DM_ERR_CUDA; \
+    } while (0)
+
+int check_launch(dm_plan* p, int n = 1)
+{
+    p->launches += n;
+    return cudaGetLastError() == cudaSuccess ? DM_OK : DM_ERR_CUDA;
+}
+
+void stage_begin(dm_plan* p, int s)
+{
+    cudaEventRecord(p->ev[2 * s], p->stream);
+}
+void stage_end(dm_plan* p, int s)
+{
+    cudaEventRecord(p->ev[2 * s + 1], p->stream);
+    p->stage_ran[s] = true;
+}
+void stage_reset(dm_plan* p)
+{
+    for (int s = 0; s < 4; ++s) p->stage_ran[s] = false;
+}
+
+int backward_splits(const dm_plan* p, int* rows_per_split)
+{
+    // enough (triangle-block x k-split) CTAs to fill the machine several times over
+    const int n_rows = (p->ix_end - p->ix_begin) * p->gd.ny;
+    const int tri_blocks = (p->n_faces + 127) / 128;
+    int want = (p->n_sm * 16 + tri_blocks - 1) / tri_blocks;
+    if (want < 1) want = 1;
+    if (want > n_rows) want = n_rows;
+    if (want > p->n_split_max) want = p->n_split_max;
+    const int rps = (n_rows + want - 1) / want;
+    *rows_per_split = rps;
+    return (n_rows + rps - 1) / rps;
+}
+
+int make_psf(const dm_plan* p, const float* cov, DmPsfDev* out)
+{
+    if (!cov) return DM_ERR_INVALID_ARG;
+    for (int i = 0; i < 6; ++i) {
+        if (!std::isfinite(cov[i])) return DM_ERR_INVALID_ARG;
+        out->cov[i] = cov[i];
+    }
+    for (int d = 0; d < 3; ++d)
+        out->org_turns[d] = (double)p->grid.origin[d] / ((double)p->grid.n[d] * (double)p->grid.spacing[d]);
+    out->inv_voxel = (float)(1.0 / ((double)p->grid.spacing[0] * p->grid.spacing[1] * p->grid.spacing[2] *
+                                    (double)p->grid.n[0] * p->grid.n[1] * p->grid.n[2]));
+    return DM_OK;
+}
+
+int ensure_fft(dm_plan* p)
+{
+    if (p->have_fft) return DM_OK;
+    const int nx = p->gd.nx, ny = p->gd.ny, nz = p->gd.nz, nzh = p->gd.nzh;
+    // inverse = 2D C2C over (x,y) for every stored n_z, then 1D C2R along z  (same order as numpy irfftn, R13)
+    int n2[2] = {nx, ny};
+    int emb2[2] = {nx, ny};
+    if (!p->have_xy) {
+        if (cufftPlanMany(&p->fft_xy, 2, n2, emb2, nzh, 1, emb2, nzh, 1, CUFFT_C2C, nzh) != CUFFT_SUCCESS) return DM_ERR_CUFFT;
+        p->have_xy = true;
+    }
+    int n1[1] = {nz};
+    int iemb[1] = {nzh}, oemb[1] = {nz};
+    if (!p->have_z) {
+        if (cufftPlanMany(&p->fft_z, 1, n1, iemb, 1, nzh, oemb, 1, nz, CUFFT_C2R, nx * ny) != CUFFT_SUCCESS) return DM_ERR_CUFFT;
+        p->have_z = true;
+    }
+    if (!p->have_r2c) {
+        if (cufftPlan3d(&p->fft_r2c, nx, ny, nz, CUFFT_R2C) != CUFFT_SUCCESS) return DM_ERR_CUFFT;
+        p->have_r2c = true;
+    }
+    if (cufftSetStream(p->fft_xy, p->stream) != CUFFT_SUCCESS || cufftSetStream(p->fft_z, p->stream) != CUFFT_SUCCESS ||
+        cufftSetStream(p->fft_r2c, p->stream) != CUFFT_SUCCESS)
+        return DM_ERR_CUFFT;
+    if (!p->spec2 && cudaMalloc(&p->spec2, n_k_of(p) * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
+    p->have_fft = true;
+    return DM_OK;
+}
+
+int run_geometry(dm_plan* p, const float* vertices_dev)
+{
+    dm_k_geometry<<<(p->n_faces + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->gd, p->rec);
+    return check_launch(p);
+}
+
+int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
+{
+    int rc = run_geometry(p, vertices_dev);
+    if (rc) return rc;
+    const long long n_slab = (long long)(p->ix_end - p->ix_begin) * p->gd.ny * p->gd.nzh;
+    const unsigned blocks = (unsigned)((n_slab + 127) / 128);
+    dm_k_forward_robust<<<blocks, 128, 0, p->stream>>>(p->rec, p->n_faces, p->gd, p->mode, p->ix_begin, p->ix_end,
+                                                       (float2*)F_dev);
+    rc = check_launch(p);
+    if (rc) return rc;
+    if (p->ix_begin == 0) {
+        dm_k_dc_entry<<<1, 256, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode, F_dev);
+        rc = check_launch(p);
+    }
+    return rc;
+}
+
+int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, float* dv_dev)
+{
+    int rc = run_geometry(p, vertices_dev);
+    if (rc) return rc;
+    int rps = 1;
+    const int n_split = backward_splits(p, &rps);
+    dim3 grid((p->n_faces + 127) / 128, n_split);
+    dm_k_backward_robust<<<grid, 128, 0, p->stream>>>(p->rec, p->n_faces, p->gd, p->mode, p->ix_begin, p->ix_end, rps,
+                                                      (const float2*)G_dev, p->part);
+    rc = check_launch(p);
+    if (rc) return rc;
+    stage_end(p, 0);
+    stage_begin(p, 3);
+    dm_k_corner_grads<<<(p->n_faces + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode,
+                                                                       n_split, p->part, (const float2*)G_dev,
+                                                                       p->ix_begin == 0 ? 1 : 0, p->corner);
+    rc = check_launch(p);
+    if (rc) return rc;
+    dm_k_vertex_gather<<<(p->n_vertices + 127) / 128, 128, 0, p->stream>>>(p->csr_off, p->csr_corner, p->n_vertices,
+                                                                           p->corner, dv_dev);
+    rc = check_launch(p);
+    stage_end(p, 3);
+    return rc;
+}
+
+int run_spectrum_to_image(dm_plan* p, const float* F_dev, const DmPsfDev& psf, float* image_dev)
+{
+    const size_t nk = n_k_of(p);
+    stage_begin(p, 1);
+    dm_k_psf_multiply<<<(unsigned)((nk + 255) / 256), 256, 0, p->stream>>>((const float2*)F_dev, p->gd, psf, p->spec);
+    int rc = check_launch(p);
+    stage_end(p, 1);
+    if (rc) return rc;
+    stage_begin(p, 2);
+    if (cufftExecC2C(p->fft_xy, (cufftComplex*)p->spec, (cufftComplex*)p->spec, CUFFT_INVERSE) != CUFFT_SUCCESS)
+        return DM_ERR_CUFFT;
+    dm_k_drop_selfconj_imag<<<(p->gd.nx * p->gd.ny + 255) / 256, 256, 0, p->stream>>>(p->spec, p->gd);
+    rc = check_launch(p);
+    if (rc) return rc;
+    if (cufftExecC2R(p->fft_z, (cufftComplex*)p->spec, image_dev) != CUFFT_SUCCESS) return DM_ERR_CUFFT;
+    stage_end(p, 2);
+    return DM_OK;
+}
+
+int run_image_to_cotangent(dm_plan* p, const float* dimage_dev, const DmPsfDev& psf, float* G_dev)
+{
+    const size_t nk = n_k_of(p);
+    stage_begin(p, 2);
+    if (cufftExecR2C(p->fft_r2c, (cufftReal*)dimage_dev, (cufftComplex*)p->spec) != CUFFT_SUCCESS) return DM_ERR_CUFFT;
+    stage_end(p, 2);
+    stage_begin(p, 1);
+    dm_k_psf_adjoint<<<(unsigned)((nk + 255) / 256), 256, 0, p->stream>>>(p->spec, p->gd, psf, (float2*)G_dev);
+    int rc = check_launch(p);
+    stage_end(p, 1);
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int dm_version(void) { return DM_VERSION; }
+
+const char* dm_error_string(int code)
+{
+    const int i = -code;
+    return (i >= 0 && i <= 6) ? kErr[i] : "unknown error";
+}
+
+int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_vertices, int32_t n_faces,
+                   const int32_t* faces_dev, void* cuda_stream)
+{
+    if (!out) return DM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!grid || !faces_dev || n_vertices <= 0 || n_faces <= 0 || (mode != DM_VOLUME && mode != DM_SURFACE))
+        return DM_ERR_INVALID_ARG;
+    for (int d = 0; d < 3; ++d)
+        if (grid->n[d] <= 0 || grid->n[d] > 4096 || !(grid->spacing[d] > 0.f) || !std::isfinite(grid->spacing[d]) ||
+            !std::isfinite(grid->origin[d]))
+            return DM_ERR_INVALID_ARG;
+    if (grid->n[2] % 2 != 0) return DM_ERR_INVALID_ARG;
+    if ((long long)n_faces * 3 > 0x7fffffffLL) return DM_ERR_INVALID_ARG;
+
+    dm_plan* p = new (std::nothrow) dm_plan();
+    if (!p) return DM_ERR_ALLOC;
+    p->grid = *grid;
+    p->mode = mode;
+    p->n_vertices = n_vertices;
+    p->n_faces = n_faces;
+    p->stream = (cudaStream_t)cuda_stream;
+    p->gd.nx = grid->n[0];
+    p->gd.ny = grid->n[1];
+    p->gd.nz = grid->n[2];
+    p->gd.nzh = grid->n[2] / 2 + 1;
+    for (int d = 0; d < 3; ++d) {
+        const double L = (double)grid->n[d] * (double)grid->spacing[d];
+        p->gd.kstep[d] = (float)(2.0 * M_PI / L);
+        p->gd.inv_len[d] = 1.0 / L;
+    }
+    p->ix_begin = 0;
+    p->ix_end = p->gd.nx;
+
+    int rc = DM_OK;
+    int dev = 0;
+    std::vector<int32_t> faces_h, off, cor, fill;
+    do {
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+        try {
+            faces_h.resize((size_t)n_faces * 3);
+            off.assign((size_t)n_vertices + 1, 0);
+            cor.resize((size_t)n_faces * 3);
+        } catch (...) { rc = DM_ERR_ALLOC; break; }
+        if (cudaMemcpyAsync(faces_h.data(), faces_dev, faces_h.size() * sizeof(int32_t), cudaMemcpyDeviceToHost,
+                            p->stream) != cudaSuccess || cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+        bool bad = false;
+        for (size_t i = 0; i < faces_h.size(); ++i) {
+            const int32_t v = faces_h[i];
+            if (v < 0 || v >= n_vertices) { bad = true; break; }
+            off[(size_t)v + 1]++;
+        }
+        if (bad) { rc = DM_ERR_BAD_MESH; break; }
+        // CSR vertex -> corner (3*face+corner), ascending corner id per vertex: the vertex star v* of eq. 13
+        for (int32_t v = 0; v < n_vertices; ++v) off[(size_t)v + 1] += off[v];
+        try { fill.assign(off.begin(), off.end() - 1); } catch (...) { rc = DM_ERR_ALLOC; break; }
+        for (size_t i = 0; i < faces_h.size(); ++i) cor[(size_t)fill[faces_h[i]]++] = (int32_t)i;
+
+        const size_t nk = n_k_of(p);
+        p->n_split_max = 64;
+        if (cudaMalloc(&p->faces, faces_h.size() * sizeof(int32_t)) != cudaSuccess ||
+            cudaMalloc(&p->csr_off, off.size() * sizeof(int32_t)) != cudaSuccess ||
+            cudaMalloc(&p->csr_corner, cor.size() * sizeof(int32_t)) != cudaSuccess ||
+            cudaMalloc(&p->rec, (size_t)n_faces * 4 * sizeof(float4)) != cudaSuccess ||
+            cudaMalloc(&p->part, (size_t)p->n_split_max * DM_BWD_NSUM * n_faces * sizeof(float)) != cudaSuccess ||
+            cudaMalloc(&p->corner, (size_t)n_faces * 9 * sizeof(float)) != cudaSuccess ||
+            cudaMalloc(&p->spec, nk * sizeof(float2)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
+        if (cudaMemcpyAsync(p->faces, faces_h.data(), faces_h.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+            cudaMemcpyAsync(p->csr_off, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+            cudaMemcpyAsync(p->csr_corner, cor.data(), cor.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+            cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+        bool ok = true;
+        for (int i = 0; i < 8; ++i) ok = ok && (cudaEventCreate(&p->ev[i]) == cudaSuccess);
+        if (!ok) { rc = DM_ERR_CUDA; break; }
+        p->ev_ok = true;
+    } while (0);
+    if (rc != DM_OK) {
+        dm_plan_destroy(p);
+        cudaGetLastError();
+        return rc;
+    }
+    *out = p;
+    return DM_OK;
+}
+
+int dm_plan_set_slab(dm_plan* p, int32_t ix_begin, int32_t ix_end)
+{
+    if (!p || ix_begin < 0 || ix_end > p->gd.nx || ix_begin >= ix_end) return DM_ERR_INVALID_ARG;
+    p->ix_begin = ix_begin;
+    p->ix_end = ix_end;
+    return DM_OK;
+}
+
+int dm_mesh_ft_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
+{
+    if (!p || !vertices_dev || !F_dev) return DM_ERR_INVALID_ARG;
+    stage_reset(p);
+    stage_begin(p, 0);
+    const int rc = run_forward(p, vertices_dev, F_dev);
+    stage_end(p, 0);
+    return rc;
+}
+
+int dm_mesh_ft_backward(dm_plan* p, const float* vertices_dev, const float* dL_dF_dev, float* dL_dvertices_dev)
+{
+    if (!p || !vertices_dev || !dL_dF_dev || !dL_dvertices_dev) return DM_ERR_INVALID_ARG;
+    stage_reset(p);
+    stage_begin(p, 0);
+    return run_backward(p, vertices_dev, dL_dF_dev, dL_dvertices_dev);
+}
+
+int dm_spectrum_to_image(dm_plan* p, const float* F_dev, const float* psf_cov_host, float* image_dev)
+{
+    if (!p || !F_dev || !image_dev) return DM_ERR_INVALID_ARG;
+    DmPsfDev psf;
+    int rc = make_psf(p, psf_cov_host, &psf);
+    if (rc) return rc;
+    if ((rc = ensure_fft(p))) return rc;
+    stage_reset(p);
+    return run_spectrum_to_image(p, F_dev, psf, image_dev);
+}
+
+int dm_image_to_spectrum_cotangent(dm_plan* p, const float* dL_dimage_dev, const float* psf_cov_host, float* G_dev)
+{
+    if (!p || !dL_dimage_dev || !G_dev) return DM_ERR_INVALID_ARG;
+    DmPsfDev psf;
+    int rc = make_psf(p, psf_cov_host, &psf);
+    if (rc) return rc;
+    if ((rc = ensure_fft(p))) return rc;
+    stage_reset(p);
+    return run_image_to_cotangent(p, dL_dimage_dev, psf, G_dev);
+}
+
+int dm_render(dm_plan* p, const float* vertices_dev, const float* psf_cov_host, float* image_dev)
+{
+    if (!p || !vertices_dev || !image_dev) return DM_ERR_INVALID_ARG;
+    if (p->ix_begin != 0 || p->ix_end != p->gd.nx) return DM_ERR_INVALID_ARG;
+    DmPsfDev psf;
+    int rc = make_psf(p, psf_cov_host, &psf);
+    if (rc) return rc;
+    if ((rc = ensure_fft(p))) return rc;
+    stage_reset(p);
+    stage_begin(p, 0);
+    rc = run_forward(p, vertices_dev, (float*)p->spec2);
+    stage_end(p, 0);
+    if (rc) return rc;
+    return run_spectrum_to_image(p, (const float*)p->spec2, psf, image_dev);
+}
+
+int dm_render_backward(dm_plan* p, const float* vertices_dev, const float* psf_cov_host, const float* dL_dimage_dev,
+                       float* dL_dvertices_dev, float* dL_dpsf_cov_host)
+{
+    if (!p || !vertices_dev || !dL_dimage_dev || !dL_dvertices_dev) return DM_ERR_INVALID_ARG;
+    if (dL_dpsf_cov_host) return DM_ERR_UNSUPPORTED;
+    if (p->ix_begin != 0 || p->ix_end != p->gd.nx) return DM_ERR_INVALID_ARG;
+    DmPsfDev psf;
+    int rc = make_psf(p, psf_cov_host, &psf);
+    if (rc) return rc;
+    if ((rc = ensure_fft(p))) return rc;
+    stage_reset(p);
+    rc = run_image_to_cotangent(p, dL_dimage_dev, psf, (float*)p->spec2);
+    if (rc) return rc;
+    stage_begin(p, 0);
+    return run_backward(p, vertices_dev, (const float*)p->spec2, dL_dvertices_dev);
+}
+
+int dm_plan_stage_ms(dm_plan* p, float ms[4])
+{
+    if (!p || !ms) return DM_ERR_INVALID_ARG;
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) return DM_ERR_CUDA;
+    for (int s = 0; s < 4; ++s) {
+        ms[s] = 0.f;
+        if (p->stage_ran[s] && cudaEventElapsedTime(&ms[s], p->ev[2 * s], p->ev[2 * s + 1]) != cudaSuccess) return DM_ERR_CUDA;
+    }
+    return DM_OK;
+}
+
+int64_t dm_plan_launch_count(const dm_plan* p) { return p ? p->launches : 0; }
+
+void dm_plan_destroy(dm_plan* p)
+{
+    if (!p) return;
+    if (p->have_xy) cufftDestroy(p->fft_xy);
+    if (p->have_z) cufftDestroy(p->fft_z);
+    if (p->have_r2c) cufftDestroy(p->fft_r2c);
+    cudaFree(p->faces);
+    cudaFree(p->csr_off);
+    cudaFree(p->csr_corner);
+    cudaFree(p->rec);
+    cudaFree(p->part);
+    cudaFree(p->corner);
+    cudaFree(p->spec);
+    cudaFree(p->spec2);
+    if (p->ev_ok)
+        for (int i = 0; i < 8; ++i) cudaEventDestroy(p->ev[i]);
+    delete p;
+}
+
+}  // extern "C"

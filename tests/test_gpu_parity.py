@@ -1,0 +1,214 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the fp64 oracle, element by element.
+
+Acceptance bars (BASELINE.json north_star):  forward max|dF| <= 1e-4 |F(0)|;  vertex gradient relative L2 <= 1e-3;
+rendered image max abs diff <= 1e-4 max|image|.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import box_mesh, build_workload, icosphere, sampled_frequencies
+from workloads.configs import image_cotangent, spectrum_cotangent
+
+pytestmark = pytest.mark.gpu
+
+FWD_TOL = 1e-4     # x |F(0)|
+GRAD_TOL = 1e-3    # relative L2
+IMG_TOL = 1e-4     # x max|image|
+
+
+@pytest.fixture(scope="module")
+def dm():
+    import torch
+    import paper_2303_10440_b200 as dm
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    dm.load_library()
+    return dm
+
+
+def _plan(dm, w, mode=None):
+    import torch
+    faces = torch.as_tensor(w.faces, device="cuda")
+    return dm.Plan(w.n, w.spacing, w.origin, w.mode if mode is None else mode, faces, w.vertices.shape[0])
+
+
+def _dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a), device="cuda")
+
+
+def _rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def _forward_full(dm, w, mode):
+    plan = _plan(dm, w, mode)
+    F = plan.mesh_ft_forward(_dev(w.vertices)).cpu().numpy()
+    ref = oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, mode)
+    return F, ref
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_forward_cfg1_full_grid(dm, mode):
+    w = build_workload(1)
+    F, ref = _forward_full(dm, w, mode)
+    assert np.isfinite(F).all()
+    err = np.abs(F - ref).max() / abs(ref[0, 0, 0])
+    assert err <= FWD_TOL, err
+    # the k = 0 entry (row A5) is the volume / area to fp32 rounding
+    assert abs(F[0, 0, 0] - ref[0, 0, 0]) <= 2e-7 * abs(ref[0, 0, 0])
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_forward_box_exact_degeneracies(dm, mode):
+    """Axis-aligned box on its own lattice: a=b and a=b=c hold exactly for axis-aligned k (eq. 15/16 cases), and
+    the ragged grid (24x20x18, not a multiple of any tile) exercises the tails."""
+    c = np.array([0.05, -0.02, 0.1])
+    h = np.array([0.2, 0.15, 0.1])
+    v, f = box_mesh(c, h)
+    n = (24, 20, 18)
+    spacing = (1 / 24, 1 / 20, 1 / 18)
+    import torch
+    plan = dm.Plan(n, spacing, (0, 0, 0), mode, torch.as_tensor(f, device="cuda"), v.shape[0])
+    v32 = v.astype(np.float32)
+    F = plan.mesh_ft_forward(_dev(v32)).cpu().numpy()
+    ref = oracle.mesh_ft_forward_grid(v32, f, n, spacing, mode)
+    assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0])
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_forward_cfg2_shape_reduced_grid(dm, mode):
+    """cfg-2 mesh (5120 perturbed triangles: several triangle tiles + tail) on a 24x24x24 grid the oracle finishes
+    in seconds."""
+    w = build_workload(2, grid_override=(24, 24, 24))
+    F, ref = _forward_full(dm, w, mode)
+    assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0])
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_forward_anisotropic_offcentre(dm, mode):
+    """Off-centre mesh partly outside the box on an anisotropic grid with L != 1 (exact phase reduction must use
+    v/L mod 1, reading R10)."""
+    v, f = icosphere(2, 0.45, (0.5, -0.3, 0.2))
+    v32 = v.astype(np.float32)
+    n = (16, 12, 20)
+    spacing = (0.11, 0.13, 0.07)
+    import torch
+    plan = dm.Plan(n, spacing, (-0.8, -0.7, -0.6), mode, torch.as_tensor(f, device="cuda"), v.shape[0])
+    F = plan.mesh_ft_forward(_dev(v32)).cpu().numpy()
+    ref = oracle.mesh_ft_forward_grid(v32, f, n, spacing, mode)
+    assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0])
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_backward_cfg1_full_grid(dm, mode):
+    w = build_workload(1)
+    G = spectrum_cotangent(w)
+    plan = _plan(dm, w, mode)
+    dv = plan.mesh_ft_backward(_dev(w.vertices), _dev(G)).cpu().numpy()
+    ref = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, mode, G.astype(np.complex128))
+    assert np.isfinite(dv).all()
+    assert _rel_l2(dv, ref) <= GRAD_TOL
+    # run-to-run bitwise reproducibility (atomic-free reduction + CSR gather, reading R22)
+    dv2 = plan.mesh_ft_backward(_dev(w.vertices), _dev(G)).cpu().numpy()
+    assert np.array_equal(dv, dv2)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_backward_identity_P9(dm, mode):
+    """sum_v dL/dv = sum_k Re(conj(G) (-i k) F(k)) -- exact identity, all on the GPU results (pin P9)."""
+    w = build_workload(2, grid_override=(16, 16, 16))
+    G = spectrum_cotangent(w)
+    plan = _plan(dm, w, mode)
+    vd = _dev(w.vertices)
+    F = plan.mesh_ft_forward(vd).cpu().numpy().astype(np.complex128)
+    dv = plan.mesh_ft_backward(vd, _dev(G)).cpu().numpy().astype(np.float64)
+    k = oracle.frequency_grid(w.n, w.spacing)
+    rhs = np.einsum("xyz,xyzd->d", np.real(np.conj(G.astype(np.complex128)) * (-1j) * F), k)
+    scale = np.abs(dv).sum(axis=0)
+    assert np.all(np.abs(dv.sum(axis=0) - rhs) <= 1e-4 * scale)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_backward_cfg2_shape_reduced_grid(dm, mode):
+    w = build_workload(2, grid_override=(16, 16, 16))
+    G = spectrum_cotangent(w)
+    plan = _plan(dm, w, mode)
+    dv = plan.mesh_ft_backward(_dev(w.vertices), _dev(G)).cpu().numpy()
+    ref = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, mode, G.astype(np.complex128))
+    assert _rel_l2(dv, ref) <= GRAD_TOL
+
+
+def test_slab_partition_matches_whole_grid(dm):
+    """Two x-slabs reproduce the whole-grid forward bit for bit and their partial gradients add up."""
+    w = build_workload(1)
+    G = spectrum_cotangent(w)
+    vd, Gd = _dev(w.vertices), _dev(G)
+    plan = _plan(dm, w)
+    F = plan.mesh_ft_forward(vd).clone()
+    dv = plan.mesh_ft_backward(vd, Gd).cpu().numpy()
+    import torch
+    F2 = torch.zeros_like(F)
+    parts = []
+    for lo, hi in ((0, 13), (13, 32)):
+        plan.set_slab(lo, hi)
+        plan.mesh_ft_forward(vd, out=F2)
+        parts.append(plan.mesh_ft_backward(vd, Gd).cpu().numpy())
+    assert torch.equal(F, F2)
+    assert _rel_l2(parts[0] + parts[1], dv) <= 1e-5
+
+
+def test_render_and_backward_cfg1(dm):
+    w = build_workload(1)
+    plan = _plan(dm, w)
+    vd = _dev(w.vertices)
+    img = plan.render(vd, w.psf_cov).cpu().numpy()
+    ref = oracle.render(w.vertices, w.faces, w.n, w.spacing, w.origin, w.psf_cov.astype(np.float64), w.mode)
+    assert np.abs(img - ref).max() <= IMG_TOL * np.abs(ref).max()
+    gi = image_cotangent(w)
+    dv = plan.render_backward(vd, w.psf_cov, _dev(gi)).cpu().numpy()
+    dref = oracle.render_backward(w.vertices, w.faces, w.n, w.spacing, w.origin, w.psf_cov.astype(np.float64), w.mode, gi)
+    assert _rel_l2(dv, dref) <= GRAD_TOL
+    ms = plan.stage_ms()
+    assert ms["mesh_ft"] > 0 and ms["fft"] > 0 and ms["psf"] > 0 and ms["scatter"] > 0
+
+
+def test_inverse_transform_semantics_R13(dm):
+    """spectrum_to_image on a deliberately NON-Hermitian half spectrum equals numpy irfftn (reading R13), and
+    image_to_spectrum_cotangent is its adjoint on independent stored entries (pin P11, reading R14)."""
+    import torch
+    n = (12, 10, 8)
+    spacing = (0.1, 0.12, 0.09)
+    origin = (-0.55, -0.6, -0.3)
+    cov = [0.02, 0.03, 0.015, 0.004, -0.003, 0.002]
+    v, f = icosphere(0, 0.3)
+    plan = dm.Plan(n, spacing, origin, 0, torch.as_tensor(f, device="cuda"), v.shape[0])
+    rng = np.random.default_rng(5)
+    shape = (n[0], n[1], n[2] // 2 + 1)
+    F = (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)).astype(np.complex64)
+    img = plan.spectrum_to_image(_dev(F), cov).cpu().numpy()
+    ref = oracle.spectrum_to_image(F, n, spacing, origin, cov)
+    assert np.abs(img - ref).max() <= 1e-5 * np.abs(ref).max()
+    y = rng.standard_normal(n).astype(np.float32)
+    Gy = plan.image_to_spectrum_cotangent(_dev(y), cov).cpu().numpy()
+    Gref = oracle.image_to_spectrum_cotangent(y, n, spacing, origin, cov)
+    assert np.abs(Gy - Gref).max() <= 1e-5 * np.abs(Gref).max()
+    lhs = float((img.astype(np.float64) * y).sum())
+    rhs = float(np.real(np.conj(Gy.astype(np.complex128)) * F).sum())
+    assert abs(lhs - rhs) <= 1e-4 * max(abs(lhs), 1.0)
+
+
+def test_error_codes(dm):
+    import torch
+    v, f = icosphere(0, 0.3)
+    bad = f.copy()
+    bad[3, 1] = 99
+    with pytest.raises(dm.DeltamicError) as e:
+        dm.Plan((8, 8, 8), (1 / 8,) * 3, (0, 0, 0), 0, torch.as_tensor(bad, device="cuda"), v.shape[0])
+    assert e.value.code == -2
+    with pytest.raises(dm.DeltamicError) as e:
+        dm.Plan((8, 8, 7), (1 / 8,) * 3, (0, 0, 0), 0, torch.as_tensor(f, device="cuda"), v.shape[0])
+    assert e.value.code == -1
+    plan = dm.Plan((8, 8, 8), (1 / 8,) * 3, (0, 0, 0), 0, torch.as_tensor(f, device="cuda"), v.shape[0])
+    with pytest.raises(dm.DeltamicError):
+        plan.set_slab(4, 4)
