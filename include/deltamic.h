@@ -76,6 +76,15 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
  * DESIGN.md section 9).  Default: the whole grid.  dm_render* require the whole grid. */
 int dm_plan_set_slab(dm_plan* plan, int32_t ix_begin, int32_t ix_end);
 
+/* Tuning / debugging knobs.  Defaults are the product path; the "robust" paths evaluate EVERY pair through the
+ * series / far-pair branches (slow, used by the tests to cross-check the fast kernels at full size). */
+typedef enum dm_option {
+    DM_OPT_FORWARD_PATH  = 0, /* 0 = fast strip kernel (default), 1 = robust per-triangle kernel                  */
+    DM_OPT_BACKWARD_PATH = 1, /* 0 = fast kernel (default), 1 = robust kernel                                     */
+    DM_OPT_TAU           = 2  /* gap-product threshold below which a pair leaves the fast path (default 1e-2)     */
+} dm_option;
+int dm_plan_set_option(dm_plan* plan, int option, double value);
+
 /* Mesh Fourier transform (the hot path, forward).
  *   surface: F(k) = sum_T 2 A_T f_T(k),  f_T = eq. 9, evaluated through a numerically
  *            stable branch (series / divided differences) where the denominators of eq. 9 vanish or nearly

@@ -6,6 +6,9 @@ streams.  There is no CPU fallback: importing the binding without the built libr
 device, raises.
 """
 from ._binding import (  # noqa: F401
+    DM_OPT_BACKWARD_PATH,
+    DM_OPT_FORWARD_PATH,
+    DM_OPT_TAU,
     DM_SURFACE,
     DM_VOLUME,
     DeltamicError,

@@ -11,7 +11,8 @@
 #include <vector>
 
 #include "../../include/deltamic.h"
-#include "dm_kernels.cuh"
+#include "dm_fast.cuh"
+#include "dm_strips.h"
 
 #define DM_VERSION 100
 
@@ -33,6 +34,15 @@ struct dm_plan {
     float2* spec = nullptr;          // [n_k] scratch spectrum (S, R or G)
     float2* spec2 = nullptr;         // [n_k] F or G inside dm_render*
     int n_split_max = 0;
+    // strip walk of the fast forward kernel (topology only; built at create)
+    int32_t *st_new = nullptr, *st_prev = nullptr, *st_ret = nullptr, *st_fid = nullptr, *st_chunk_off = nullptr;
+    int st_n_rec = 0, st_n_chunks = 0;
+    float4* st_rec = nullptr;        // [st_n_rec*3] strip records (A1)
+    float2* fwd_part = nullptr;      // [st_n_chunks * n_k] per-chunk partial spectra
+    unsigned int* hmax2 = nullptr;   // longest squared edge (float bits), rebuilt every call
+    double* dc_part = nullptr;       // [DM_DC_BLOCKS] block sums of the k = 0 entry
+    int fwd_path = 0, bwd_path = 1;  // 0 = fast, 1 = robust
+    float tau = 1e-2f;
     cufftHandle fft_xy = 0, fft_z = 0, fft_r2c = 0;
     bool have_xy = false, have_z = false, have_r2c = false, have_fft = false;
     // stage timing
@@ -137,7 +147,7 @@ int run_geometry(dm_plan* p, const float* vertices_dev)
     return check_launch(p);
 }
 
-int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
+int run_forward_robust(dm_plan* p, const float* vertices_dev, float* F_dev)
 {
     int rc = run_geometry(p, vertices_dev);
     if (rc) return rc;
@@ -145,10 +155,51 @@ int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
     const unsigned blocks = (unsigned)((n_slab + 127) / 128);
     dm_k_forward_robust<<<blocks, 128, 0, p->stream>>>(p->rec, p->n_faces, p->gd, p->mode, p->ix_begin, p->ix_end,
                                                        (float2*)F_dev);
-    rc = check_launch(p);
+    return check_launch(p);
+}
+
+int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
+{
+    if (cudaMemsetAsync(p->hmax2, 0, sizeof(unsigned int), p->stream) != cudaSuccess) return DM_ERR_CUDA;
+    DmStripDev st = {p->st_new, p->st_prev, p->st_ret, p->st_fid, p->st_n_rec};
+    dm_k_strip_geometry<<<(p->st_n_rec + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, st, p->gd, p->mode,
+                                                                           p->st_rec, p->hmax2);
+    int rc = check_launch(p);
+    if (rc) return rc;
+    const int n_yruns = (p->gd.ny + DM_K - 1) / DM_K;
+    const long long n_thr = (long long)(p->ix_end - p->ix_begin) * n_yruns * p->gd.nzh;
+    dim3 grid((unsigned)((n_thr + DM_FAST_THREADS - 1) / DM_FAST_THREADS), (unsigned)p->st_n_chunks);
+    const size_t stride = n_k_of(p);
+    if (p->mode == DM_SURFACE)
+        dm_k_forward_fast<1><<<grid, DM_FAST_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->gd, p->ix_begin, p->ix_end,
+                                                                      n_yruns, p->tau, p->hmax2, stride, p->fwd_part);
+    else
+        dm_k_forward_fast<0><<<grid, DM_FAST_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->gd, p->ix_begin, p->ix_end,
+                                                                      n_yruns, p->tau, p->hmax2, stride, p->fwd_part);
+    if ((rc = check_launch(p))) return rc;
+    const int W = 2 * DM_LOWK_BOX + 1;
+    const unsigned lowk_blocks = (unsigned)((W * W * (DM_LOWK_BOX + 1) + 3) / 4);
+    if (p->mode == DM_SURFACE)
+        dm_k_forward_lowk<1><<<lowk_blocks, 128, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
+                                                                 p->ix_end, p->hmax2, (float2*)F_dev);
+    else
+        dm_k_forward_lowk<0><<<lowk_blocks, 128, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
+                                                                 p->ix_end, p->hmax2, (float2*)F_dev);
+    if ((rc = check_launch(p))) return rc;
+    const long long n_slab = (long long)(p->ix_end - p->ix_begin) * p->gd.ny * p->gd.nzh;
+    dm_k_forward_finish<<<(unsigned)((n_slab + 255) / 256), 256, 0, p->stream>>>(p->fwd_part, stride, p->st_n_chunks, p->gd,
+                                                                                p->ix_begin, p->ix_end, p->hmax2, (float2*)F_dev);
+    return check_launch(p);
+}
+
+int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
+{
+    int rc = p->fwd_path == 0 ? run_forward_fast(p, vertices_dev, F_dev) : run_forward_robust(p, vertices_dev, F_dev);
     if (rc) return rc;
     if (p->ix_begin == 0) {
-        dm_k_dc_entry<<<1, 256, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode, F_dev);
+        dm_k_dc_partial<<<DM_DC_BLOCKS, 256, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode, p->dc_part);
+        if ((rc = check_launch(p))) return rc;
+        dm_k_dc_final<<<1, DM_DC_BLOCKS, 0, p->stream>>>(p->dc_part, F_dev);
         rc = check_launch(p);
     }
     return rc;
@@ -255,6 +306,9 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
     }
     p->ix_begin = 0;
     p->ix_end = p->gd.nx;
+    // gap-product threshold of the fast path: one excluded-or-not pair may cost ~1e-6 (sum|d|)/tau of ONE triangle's
+    // weight, i.e. ~1/(n_T tau) 1e-5 of |F(0)|; DESIGN.md section 6
+    p->tau = (float)std::min(1e-2, std::max(2e-5, 2.0 / (double)n_faces));
 
     int rc = DM_OK;
     int dev = 0;
@@ -294,6 +348,34 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
             cudaMemcpyAsync(p->csr_off, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
             cudaMemcpyAsync(p->csr_corner, cor.data(), cor.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
             cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+        // strip walk for the fast forward kernel; chunks so that (k-blocks x chunks) fills the machine several times
+        {
+            const int n_yruns = (p->gd.ny + DM_K - 1) / DM_K;
+            const long long kblocks = ((long long)p->gd.nx * n_yruns * p->gd.nzh + DM_FAST_THREADS - 1) / DM_FAST_THREADS;
+            const long long slots = (long long)p->n_sm * 4;
+            long long want = (6 * slots + kblocks - 1) / kblocks;
+            want = std::min<long long>(want, std::max<long long>(1, n_faces / 1536));
+            want = std::max<long long>(1, std::min<long long>(want, 64));
+            DmStripRecords sr;
+            try { sr = dm_build_strips(faces_h.data(), n_faces, n_vertices, (int)want); } catch (...) { rc = DM_ERR_ALLOC; break; }
+            p->st_n_rec = (int)sr.fid.size();
+            p->st_n_chunks = (int)sr.chunk_off.size() - 1;
+            const size_t nb = (size_t)p->st_n_rec * sizeof(int32_t);
+            if (cudaMalloc(&p->st_new, nb) != cudaSuccess || cudaMalloc(&p->st_prev, nb) != cudaSuccess ||
+                cudaMalloc(&p->st_ret, nb) != cudaSuccess || cudaMalloc(&p->st_fid, nb) != cudaSuccess ||
+                cudaMalloc(&p->st_chunk_off, sr.chunk_off.size() * sizeof(int32_t)) != cudaSuccess ||
+                cudaMalloc(&p->st_rec, (size_t)p->st_n_rec * 3 * sizeof(float4)) != cudaSuccess ||
+                cudaMalloc(&p->fwd_part, (size_t)p->st_n_chunks * nk * sizeof(float2)) != cudaSuccess ||
+                cudaMalloc(&p->hmax2, sizeof(unsigned int)) != cudaSuccess ||
+                cudaMalloc(&p->dc_part, DM_DC_BLOCKS * sizeof(double)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
+            if (cudaMemcpyAsync(p->st_new, sr.vid_new.data(), nb, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+                cudaMemcpyAsync(p->st_prev, sr.vid_prev.data(), nb, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+                cudaMemcpyAsync(p->st_ret, sr.vid_ret.data(), nb, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+                cudaMemcpyAsync(p->st_fid, sr.fid.data(), nb, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+                cudaMemcpyAsync(p->st_chunk_off, sr.chunk_off.data(), sr.chunk_off.size() * sizeof(int32_t),
+                                cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+                cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+        }
         bool ok = true;
         for (int i = 0; i < 8; ++i) ok = ok && (cudaEventCreate(&p->ev[i]) == cudaSuccess);
         if (!ok) { rc = DM_ERR_CUDA; break; }
@@ -314,6 +396,28 @@ int dm_plan_set_slab(dm_plan* p, int32_t ix_begin, int32_t ix_end)
     p->ix_begin = ix_begin;
     p->ix_end = ix_end;
     return DM_OK;
+}
+
+int dm_plan_set_option(dm_plan* p, int option, double value)
+{
+    if (!p) return DM_ERR_INVALID_ARG;
+    switch (option) {
+        case DM_OPT_FORWARD_PATH:
+            if (value != 0.0 && value != 1.0) return DM_ERR_INVALID_ARG;
+            p->fwd_path = (int)value;
+            return DM_OK;
+        case DM_OPT_BACKWARD_PATH:
+            if (value != 0.0 && value != 1.0) return DM_ERR_INVALID_ARG;
+            if (value == 0.0) return DM_ERR_UNSUPPORTED;
+            p->bwd_path = (int)value;
+            return DM_OK;
+        case DM_OPT_TAU:
+            if (!(value >= 0.0) || !std::isfinite(value)) return DM_ERR_INVALID_ARG;
+            p->tau = (float)value;
+            return DM_OK;
+        default:
+            return DM_ERR_INVALID_ARG;
+    }
 }
 
 int dm_mesh_ft_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
@@ -416,6 +520,15 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->corner);
     cudaFree(p->spec);
     cudaFree(p->spec2);
+    cudaFree(p->st_new);
+    cudaFree(p->st_prev);
+    cudaFree(p->st_ret);
+    cudaFree(p->st_fid);
+    cudaFree(p->st_chunk_off);
+    cudaFree(p->st_rec);
+    cudaFree(p->fwd_part);
+    cudaFree(p->hmax2);
+    cudaFree(p->dc_part);
     if (p->ev_ok)
         for (int i = 0; i < 8; ++i) cudaEventDestroy(p->ev[i]);
     delete p;

@@ -47,13 +47,15 @@ __global__ void dm_k_geometry(const float* __restrict__ vertices, const int32_t*
 }
 
 // ---- A5: the k = 0 entry in fp64: volume 1/6 sum v1.(v2 x v3), or total area sum |m_T|/2 -------------------------
-// One block, fixed-order tree reduction: deterministic.
-__global__ void dm_k_dc_entry(const float* __restrict__ vertices, const int32_t* __restrict__ faces, int n_faces,
-                              int mode, float* __restrict__ F0)
+// Two stages, both with fixed-order tree reductions (deterministic): DM_DC_BLOCKS block sums, then one final block.
+#define DM_DC_BLOCKS 64
+__global__ void __launch_bounds__(256)
+dm_k_dc_partial(const float* __restrict__ vertices, const int32_t* __restrict__ faces, int n_faces, int mode,
+                double* __restrict__ partial)
 {
     __shared__ double sh[256];
     double acc = 0.0;
-    for (int t = threadIdx.x; t < n_faces; t += blockDim.x) {
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n_faces; t += gridDim.x * blockDim.x) {
         const int i1 = faces[3 * t], i2 = faces[3 * t + 1], i3 = faces[3 * t + 2];
         const double a[3] = {vertices[3 * i1], vertices[3 * i1 + 1], vertices[3 * i1 + 2]};
         const double b[3] = {vertices[3 * i2], vertices[3 * i2 + 1], vertices[3 * i2 + 2]};
@@ -70,6 +72,18 @@ __global__ void dm_k_dc_entry(const float* __restrict__ vertices, const int32_t*
     sh[threadIdx.x] = acc;
     __syncthreads();
     for (int s = blockDim.x / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+__global__ void __launch_bounds__(DM_DC_BLOCKS)
+dm_k_dc_final(const double* __restrict__ partial, float* __restrict__ F0)
+{
+    __shared__ double sh[DM_DC_BLOCKS];
+    sh[threadIdx.x] = partial[threadIdx.x];
+    __syncthreads();
+    for (int s = DM_DC_BLOCKS / 2; s > 0; s >>= 1) {
         if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
         __syncthreads();
     }
