@@ -81,7 +81,8 @@ int dm_plan_set_slab(dm_plan* plan, int32_t ix_begin, int32_t ix_end);
 typedef enum dm_option {
     DM_OPT_FORWARD_PATH  = 0, /* 0 = fast strip kernel (default), 1 = robust per-triangle kernel                  */
     DM_OPT_BACKWARD_PATH = 1, /* 0 = fast kernel (default), 1 = robust kernel                                     */
-    DM_OPT_TAU           = 2  /* gap-product threshold below which a pair leaves the fast path (default 1e-2)     */
+    DM_OPT_TAU           = 2, /* forward: gap-product threshold |pqr| below which a pair leaves the fast path       */
+    DM_OPT_TAU_BWD       = 3  /* backward: threshold on min|gap| * |pqr| below which a pair leaves the fast path      */
 } dm_option;
 int dm_plan_set_option(dm_plan* plan, int option, double value);
 

@@ -12,6 +12,7 @@
 
 #include "../../include/deltamic.h"
 #include "dm_fast.cuh"
+#include "dm_bwd_fast.cuh"
 #include "dm_strips.h"
 
 #define DM_VERSION 100
@@ -29,6 +30,7 @@ struct dm_plan {
     int32_t* csr_off = nullptr;      // [n_vertices+1]
     int32_t* csr_corner = nullptr;   // [n_faces*3]   3*face+corner, ascending per vertex
     float4* rec = nullptr;           // [n_faces*4]   triangle records (A1)
+    float4* brec = nullptr;          // [n_faces*DM_BF_REC] backward triangle records (A1)
     float* part = nullptr;           // [n_split_max*13*n_faces]
     float* corner = nullptr;         // [n_faces*9]
     float2* spec = nullptr;          // [n_k] scratch spectrum (S, R or G)
@@ -41,8 +43,8 @@ struct dm_plan {
     float2* fwd_part = nullptr;      // [st_n_chunks * n_k] per-chunk partial spectra
     unsigned int* hmax2 = nullptr;   // longest squared edge (float bits), rebuilt every call
     double* dc_part = nullptr;       // [DM_DC_BLOCKS] block sums of the k = 0 entry
-    int fwd_path = 0, bwd_path = 1;  // 0 = fast, 1 = robust
-    float tau = 1e-2f;
+    int fwd_path = 0, bwd_path = 0;  // 0 = fast, 1 = robust
+    float tau = 1e-2f, tau_b = 2e-3f;
     cufftHandle fft_xy = 0, fft_z = 0, fft_r2c = 0;
     bool have_xy = false, have_z = false, have_r2c = false, have_fft = false;
     // stage timing
@@ -86,10 +88,10 @@ void stage_reset(dm_plan* p)
 
 int backward_splits(const dm_plan* p, int* rows_per_split)
 {
-    // enough (triangle-block x k-split) CTAs to fill the machine several times over
+    // enough (triangle-block x k-split) CTAs to fill the machine (4 CTAs per SM) about 12 times over: short tail
     const int n_rows = (p->ix_end - p->ix_begin) * p->gd.ny;
     const int tri_blocks = (p->n_faces + 127) / 128;
-    int want = (p->n_sm * 16 + tri_blocks - 1) / tri_blocks;
+    int want = (p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
     if (want < 1) want = 1;
     if (want > n_rows) want = n_rows;
     if (want > p->n_split_max) want = p->n_split_max;
@@ -207,13 +209,26 @@ int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
 
 int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, float* dv_dev)
 {
-    int rc = run_geometry(p, vertices_dev);
-    if (rc) return rc;
     int rps = 1;
     const int n_split = backward_splits(p, &rps);
     dim3 grid((p->n_faces + 127) / 128, n_split);
-    dm_k_backward_robust<<<grid, 128, 0, p->stream>>>(p->rec, p->n_faces, p->gd, p->mode, p->ix_begin, p->ix_end, rps,
-                                                      (const float2*)G_dev, p->part);
+    const size_t row_smem = 2 * (size_t)p->gd.nzh * sizeof(float4);
+    int rc;
+    if (p->bwd_path == 0 && row_smem <= 32 * 1024) {
+        dm_k_bwd_geometry<<<(p->n_faces + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->gd, p->brec);
+        if ((rc = check_launch(p))) return rc;
+        static_assert(DM_BF_THREADS == 128, "grid.x above assumes 128 triangles per CTA");
+        if (p->mode == DM_SURFACE)
+            dm_k_backward_fast<1><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(p->brec, p->n_faces, p->gd, p->ix_begin, p->ix_end,
+                                                                                rps, p->tau_b, (const float2*)G_dev, p->part);
+        else
+            dm_k_backward_fast<0><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(p->brec, p->n_faces, p->gd, p->ix_begin, p->ix_end,
+                                                                                rps, p->tau_b, (const float2*)G_dev, p->part);
+    } else {
+        if ((rc = run_geometry(p, vertices_dev))) return rc;
+        dm_k_backward_robust<<<grid, 128, 0, p->stream>>>(p->rec, p->n_faces, p->gd, p->mode, p->ix_begin, p->ix_end, rps,
+                                                          (const float2*)G_dev, p->part);
+    }
     rc = check_launch(p);
     if (rc) return rc;
     stage_end(p, 0);
@@ -341,6 +356,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
             cudaMalloc(&p->csr_off, off.size() * sizeof(int32_t)) != cudaSuccess ||
             cudaMalloc(&p->csr_corner, cor.size() * sizeof(int32_t)) != cudaSuccess ||
             cudaMalloc(&p->rec, (size_t)n_faces * 4 * sizeof(float4)) != cudaSuccess ||
+            cudaMalloc(&p->brec, (size_t)n_faces * DM_BF_REC * sizeof(float4)) != cudaSuccess ||
             cudaMalloc(&p->part, (size_t)p->n_split_max * DM_BWD_NSUM * n_faces * sizeof(float)) != cudaSuccess ||
             cudaMalloc(&p->corner, (size_t)n_faces * 9 * sizeof(float)) != cudaSuccess ||
             cudaMalloc(&p->spec, nk * sizeof(float2)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
@@ -408,12 +424,15 @@ int dm_plan_set_option(dm_plan* p, int option, double value)
             return DM_OK;
         case DM_OPT_BACKWARD_PATH:
             if (value != 0.0 && value != 1.0) return DM_ERR_INVALID_ARG;
-            if (value == 0.0) return DM_ERR_UNSUPPORTED;
             p->bwd_path = (int)value;
             return DM_OK;
         case DM_OPT_TAU:
             if (!(value >= 0.0) || !std::isfinite(value)) return DM_ERR_INVALID_ARG;
             p->tau = (float)value;
+            return DM_OK;
+        case DM_OPT_TAU_BWD:
+            if (!(value >= 0.0) || !std::isfinite(value)) return DM_ERR_INVALID_ARG;
+            p->tau_b = (float)value;
             return DM_OK;
         default:
             return DM_ERR_INVALID_ARG;
@@ -516,6 +535,7 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->csr_off);
     cudaFree(p->csr_corner);
     cudaFree(p->rec);
+    cudaFree(p->brec);
     cudaFree(p->part);
     cudaFree(p->corner);
     cudaFree(p->spec);

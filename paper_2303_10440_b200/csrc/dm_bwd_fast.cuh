@@ -1,0 +1,346 @@
+// dm_bwd_fast.cuh -- optimised backward mesh-FT kernel (rows A1, A6 of the hot path), sm_100a.
+//
+// Layout.  One THREAD owns one triangle and keeps its 13 k-sums in registers; a CTA of DM_BF_THREADS triangles walks a
+// range of (i_x,i_y) rows of the stored spectrum, innermost along z.  Every thread of the CTA is at the SAME frequency
+// at the same time, so everything that depends on k only -- kappa = conj(G) (surface) or i conj(G)/|k|^2 (volume), k_z --
+// is computed once per CTA and row into shared memory and read back as one broadcast LDS.128 per pair: there is no
+// reduction across threads at all (O(N n_v) backward; :182-186 eq. 13 is the later CSR gather).
+//
+// Arithmetic of the generic pair.  With nodes x_j = k.v_j, E_j = e^{-i x_j} and gaps
+// p = x_1-x_0, q = x_2-x_0, r = q-p, eq. 9 is  g = sum_j c_j E_j  with REAL coefficients
+//     c_0 = -1/(pq),  c_1 = 1/(pr),  c_2 = -1/(qr)        (one MUFU.RCP of pqr),
+// and its node derivatives (the closed form of PAPER.md:171-173 eq. 11 with reading R2, regrouped) are
+//     dg/dx_1 = sum_j al_j E_j - i c_1 E_1,   al_0 = q c_0^2, al_2 = -q c_2^2, al_1 = -al_0-al_2   (sum_j c_j = 0)
+//     dg/dx_2 = sum_j be_j E_j - i c_2 E_2,   be_0 = p c_0^2, be_1 = -p c_1^2, be_2 = -be_0-be_1
+//     dg/dx_0 = -i g - dg/dx_1 - dg/dx_2.
+// With A_j = kappa E_j the four real numbers a pair contributes are
+//     s0 = Re(kappa g) = sum c_j Re A_j,  sI = Im(kappa g) = sum c_j Im A_j,
+//     sb = Re(kappa dg/dx_1) = sum al_j Re A_j + c_1 Im A_1,   sc likewise.
+// Phases advance along z by one complex rotation per vertex (rotor e^{-i kstep_z v_z} built in fp64 by the geometry
+// pre-pass) and are re-seeded EXACTLY (32-bit integer turns) every DM_BF_SEG frequencies.
+//
+// Near-degenerate pairs (reading R4).  The derivative coefficients grow like 1/(gap^2 gap'), so a pair
+// with  min|gap| * |pqr| < tau_b  is excluded from the fast sums (its reciprocal is forced to 0) and flagged in a per-
+// thread bit mask.  After each chunk of <= DM_BF_CHUNK frequencies the WARP pools its flagged pairs in shared memory,
+// sorted by owner, and evaluates them 32 at a time, one pair per lane whatever its owner: the series branch where all
+// gaps are small, the branch-free far-pair variant otherwise.  A segmented warp scan sums the results of one owner and
+// the run's last lane adds them to that owner's shared accumulators -- a fixed order, so the result is bitwise
+// reproducible (reading R22), and the divergent work is spread evenly over the lanes.
+#pragma once
+#include "dm_kernels.cuh"
+
+#define DM_BF_THREADS 128
+#define DM_BF_SEG 32            // frequencies between exact phase re-seeds = bits of the flag mask
+#define DM_BF_REC 7             // float4 per backward triangle record
+
+// backward triangle record (7 x float4 = 112 B), rebuilt every call (row A1):
+//   r0..r2 = (u_j.xyz [uint32 bit patterns: v_j / L in fixed-point turns], -)   j = 0,1,2
+//   r3 = (eb.xyz, rho_0.re)   r4 = (ec.xyz, rho_0.im)   r5 = (m_T.xyz, |m_T|)   r6 = (rho_1.re, rho_1.im, rho_2.re, rho_2.im)
+//   eb = v_1-v_0, ec = v_2-v_0, rho_j = e^{-i kstep_z v_jz}
+__global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int32_t* __restrict__ faces, int n_faces,
+                                  DmGridDev grid, float4* __restrict__ rec)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_faces) return;
+    float v[3][3];
+    uint32_t u[3][3];
+    float rho[3][2];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const int i = faces[3 * t + j];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            v[j][d] = vertices[3 * i + d];
+            double tt = (double)v[j][d] * grid.inv_len[d];
+            tt -= floor(tt);
+            u[j][d] = (uint32_t)(unsigned long long)(tt * 4294967296.0 + 0.5);
+        }
+        double tz = (double)v[j][2] * grid.inv_len[2];
+        tz -= rint(tz);
+        double sn, cs;
+        sincospi(2.0 * tz, &sn, &cs);
+        rho[j][0] = (float)cs;
+        rho[j][1] = (float)(-sn);
+    }
+    const float eb[3] = {v[1][0] - v[0][0], v[1][1] - v[0][1], v[1][2] - v[0][2]};
+    const float ec[3] = {v[2][0] - v[0][0], v[2][1] - v[0][1], v[2][2] - v[0][2]};
+    const float m[3] = {eb[1] * ec[2] - eb[2] * ec[1], eb[2] * ec[0] - eb[0] * ec[2], eb[0] * ec[1] - eb[1] * ec[0]};
+    const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+    float4* o = rec + (size_t)DM_BF_REC * t;
+#pragma unroll
+    for (int j = 0; j < 3; ++j)
+        o[j] = make_float4(__uint_as_float(u[j][0]), __uint_as_float(u[j][1]), __uint_as_float(u[j][2]), 0.f);
+    o[3] = make_float4(eb[0], eb[1], eb[2], rho[0][0]);
+    o[4] = make_float4(ec[0], ec[1], ec[2], rho[0][1]);
+    o[5] = make_float4(m[0], m[1], m[2], mn);
+    o[6] = make_float4(rho[1][0], rho[1][1], rho[2][0], rho[2][1]);
+}
+
+
+// shared-memory queue of one warp's flagged pairs of one chunk (processed DM_BF_QCAP at a time)
+#define DM_BF_CHUNK 96          // frequencies per chunk = 3 flag words per thread
+struct DmBfQueue {
+    unsigned short code[32 * DM_BF_CHUNK];  // owner lane << 7 | frequency index inside the chunk, sorted
+};
+
+struct dm_bf_true { static constexpr bool value = true; };
+struct dm_bf_false { static constexpr bool value = false; };
+
+// what one pair adds to the row sums (plain and k_z-weighted sums of s0, sI, sb, sc)
+struct DmBfRow {
+    float S0, S0z, SI, SIz, SB, SBz, SC, SCz;
+};
+template <int MODE>
+__device__ __forceinline__ void dm_bf_add(DmBfRow& a, float kz, float om, float s0, float sI, float sb, float sc)
+{
+    if (MODE == 0) {  // volume: omega = k.m_T weights the derivative sums, Q needs k s0
+        sI *= om;
+        sb *= om;
+        sc *= om;
+        a.S0z = fmaf(kz, s0, a.S0z);
+    }
+    a.S0 += s0;
+    a.SI += sI;
+    a.SIz = fmaf(kz, sI, a.SIz);
+    a.SB += sb;
+    a.SBz = fmaf(kz, sb, a.SBz);
+    a.SC += sc;
+    a.SCz = fmaf(kz, sc, a.SCz);
+}
+
+// ---- A6 backward, fast kernel -----------------------------------------------------------------------------------
+// grid = (ceil(n_faces / DM_BF_THREADS), n_split); part[(split*13 + s)*n_faces + t] as in dm_k_backward_robust.
+// dynamic shared memory: 2 * nzh float4 (kappa.re, kappa.im, k_z, -) double-buffered rows.
+template <int MODE>
+__global__ void __launch_bounds__(DM_BF_THREADS, 4)
+dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, int ix_begin, int ix_end,
+                   int rows_per_split, float tau_b, const float2* __restrict__ G, float* __restrict__ part)
+{
+    extern __shared__ float4 dm_bf_smem[];
+    __shared__ DmBfQueue queue[DM_BF_THREADS / 32];
+    __shared__ float4 trec[DM_BF_THREADS * DM_BF_REC];   // this CTA's triangle records (the pooled path reads other lanes')
+    __shared__ float wacc[(DM_BF_THREADS / 32) * 8 * 32];  // per warp: 8 row sums x 32 owners, filled by the pooled path
+    float4* const sk = dm_bf_smem;
+    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+    const int t = blockIdx.x * DM_BF_THREADS + tid;
+    const bool live = t < n_faces;
+    const int tt = live ? t : n_faces - 1;
+#pragma unroll
+    for (int i = 0; i < DM_BF_REC; ++i) trec[tid * DM_BF_REC + i] = rec[(size_t)DM_BF_REC * tt + i];
+    const float4 r0 = trec[tid * DM_BF_REC + 0], r1 = trec[tid * DM_BF_REC + 1], r2 = trec[tid * DM_BF_REC + 2],
+                 r3 = trec[tid * DM_BF_REC + 3], r4 = trec[tid * DM_BF_REC + 4], r5 = trec[tid * DM_BF_REC + 5],
+                 r6 = trec[tid * DM_BF_REC + 6];
+    const uint32_t u0x = __float_as_uint(r0.x), u0y = __float_as_uint(r0.y), u0z = __float_as_uint(r0.z);
+    const uint32_t u1x = __float_as_uint(r1.x), u1y = __float_as_uint(r1.y), u1z = __float_as_uint(r1.z);
+    const uint32_t u2x = __float_as_uint(r2.x), u2y = __float_as_uint(r2.y), u2z = __float_as_uint(r2.z);
+    const cf rho0 = {r3.w, r4.w}, rho1 = {r6.x, r6.y}, rho2 = {r6.z, r6.w};
+    const int nzh = grid.nzh;
+    const int n_rows = (ix_end - ix_begin) * grid.ny;
+    const int row_begin = blockIdx.y * rows_per_split;
+    const int row_end = min(n_rows, row_begin + rows_per_split);
+    DmBfQueue& Q = queue[wrp];
+    const float4* const wrec = trec + wrp * 32 * DM_BF_REC;   // records of this warp's 32 triangles
+
+#pragma unroll
+    for (int i = 0; i < 8; ++i) wacc[i * DM_BF_THREADS + tid] = 0.f;
+    // acc: [0] S0 | [1..3] Q | [4..6] W | [7..9] Vb | [10..12] Vc   (dm_k_backward_robust)
+    float acc[DM_BWD_NSUM];
+#pragma unroll
+    for (int s = 0; s < DM_BWD_NSUM; ++s) acc[s] = 0.f;
+
+    // stage kappa and k_z of one row into buffer b
+    auto stage_row = [&](int row, int b) {
+        const int ix = ix_begin + row / grid.ny, iy = row % grid.ny;
+        const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
+        const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
+        const float2* Grow = G + ((size_t)ix * grid.ny + iy) * nzh;
+        for (int iz = tid; iz < nzh; iz += DM_BF_THREADS) {
+            const float kz = grid.kstep[2] * iz;
+            const float2 Gk = Grow[iz];
+            float4 o;
+            if (MODE == 1) {
+                o = make_float4(Gk.x, -Gk.y, kz, 0.f);                       // conj(G)
+            } else {
+                const float k2 = kx * kx + ky * ky + kz * kz;
+                const float inv_k2 = (k2 > 0.f) ? 1.0f / k2 : 0.f;           // k = 0 is handled by dm_k_corner_grads
+                o = make_float4(Gk.y * inv_k2, Gk.x * inv_k2, kz, 0.f);      // i conj(G) / |k|^2
+            }
+            sk[b * nzh + iz] = o;
+        }
+    };
+
+    if (row_begin < row_end) stage_row(row_begin, 0);
+    __syncthreads();
+    for (int row = row_begin; row < row_end; ++row) {
+        const int b = (row - row_begin) & 1;
+        if (row + 1 < row_end) stage_row(row + 1, b ^ 1);
+        const float4* __restrict__ skr = sk + b * nzh;
+        const int ix = ix_begin + row / grid.ny, iy = row % grid.ny;
+        const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
+        const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
+        const float prow = fmaf(kx, r3.x, ky * r3.y), qrow = fmaf(kx, r4.x, ky * r4.y);
+        const float omrow = fmaf(kx, r5.x, ky * r5.y);
+        const uint32_t tr0 = (uint32_t)nx * u0x + (uint32_t)ny * u0y, tr1 = (uint32_t)nx * u1x + (uint32_t)ny * u1y,
+                       tr2 = (uint32_t)nx * u2x + (uint32_t)ny * u2y;
+        DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+
+        for (int zc = 0; zc < nzh; zc += DM_BF_CHUNK) {
+            const int clen = min(DM_BF_CHUNK, nzh - zc);
+            uint32_t fl[DM_BF_CHUNK / DM_BF_SEG];
+            // ---- fast pass over the chunk, one exactly seeded segment at a time --------------------------------------
+#pragma unroll
+            for (int sg = 0; sg < DM_BF_CHUNK / DM_BF_SEG; ++sg) {
+                fl[sg] = 0;
+                const int z0 = zc + sg * DM_BF_SEG;
+                const int len = min(DM_BF_SEG, zc + clen - z0);
+                if (len <= 0) continue;
+                cf E0 = dm_expmi_turns(tr0 + (uint32_t)z0 * u0z), E1 = dm_expmi_turns(tr1 + (uint32_t)z0 * u1z),
+                   E2 = dm_expmi_turns(tr2 + (uint32_t)z0 * u2z);
+                uint32_t flags = 0;
+#pragma unroll 4
+                for (int j = 0; j < len; ++j) {
+                    const float4 kk = skr[z0 + j];
+                    const float kz = kk.z;
+                    const float p = fmaf(kz, r3.z, prow), q = fmaf(kz, r4.z, qrow), r = q - p;
+                    const float pqr = (p * q) * r;
+                    const float m1 = fminf(fminf(fabsf(p), fabsf(q)), fabsf(r));
+                    const bool bad = m1 * fabsf(pqr) < tau_b;
+                    flags |= (bad ? 1u : 0u) << j;
+                    const float R = bad ? 0.f : dm_rcp_approx(pqr);
+                    const float c0 = -r * R, c1 = q * R, c2 = -p * R;
+                    const float c0s = c0 * c0, c1s = c1 * c1, c2s = c2 * c2;
+                    const float a0 = q * c0s, a2 = -q * c2s, a1 = -(a0 + a2);
+                    const float b0 = p * c0s, b1 = -p * c1s, b2 = -(b0 + b1);
+                    const cf kap = {kk.x, kk.y};
+                    const cf A0 = cmul(kap, E0), A1 = cmul(kap, E1), A2 = cmul(kap, E2);
+                    const float s0 = fmaf(c0, A0.re, fmaf(c1, A1.re, c2 * A2.re));
+                    const float sI = fmaf(c0, A0.im, fmaf(c1, A1.im, c2 * A2.im));
+                    const float sb = fmaf(a0, A0.re, fmaf(a1, A1.re, fmaf(a2, A2.re, c1 * A1.im)));
+                    const float sc = fmaf(b0, A0.re, fmaf(b1, A1.re, fmaf(b2, A2.re, c2 * A2.im)));
+                    dm_bf_add<MODE>(rs, kz, fmaf(kz, r5.z, omrow), s0, sI, sb, sc);
+                    E0 = cmul(E0, rho0);
+                    E1 = cmul(E1, rho1);
+                    E2 = cmul(E2, rho2);
+                }
+                fl[sg] = live ? flags : 0u;
+            }
+            // ---- pooled slow path -------------------------------------------------------------------------------------
+            int cnt = 0;
+#pragma unroll
+            for (int sg = 0; sg < DM_BF_CHUNK / DM_BF_SEG; ++sg) cnt += __popc(fl[sg]);
+            if (__any_sync(0xffffffffu, cnt != 0)) {
+                int off = cnt;  // inclusive prefix sum over lanes
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int n = __shfl_up_sync(0xffffffffu, off, o);
+                    if (lane >= o) off += n;
+                }
+                const int total = __shfl_sync(0xffffffffu, off, 31);
+                // owners queue their pairs in (lane, frequency) order
+                int w = off - cnt;
+#pragma unroll
+                for (int sg = 0; sg < DM_BF_CHUNK / DM_BF_SEG; ++sg) {
+                    uint32_t f = fl[sg];
+                    while (f) {
+                        const int j = __ffs(f) - 1;
+                        f &= f - 1;
+                        Q.code[w++] = (unsigned short)((lane << 7) | (sg * DM_BF_SEG + j));
+                    }
+                }
+                __syncwarp();
+                // rounds of 32 queued pairs: every lane evaluates one pair; a segmented scan over the (sorted) owners sums
+                // the pairs of one owner, and the last lane of each run adds the run into the owner's shared accumulators
+                for (int base = 0; base < total; base += 32) {
+                    const int e = base + lane;
+                    const bool have = e < total;
+                    const int code = have ? Q.code[e] : 0;
+                    const int ol = have ? (code >> 7) : -1 - lane, jz = zc + (code & 127);
+                    const float4* orc = wrec + (code >> 7) * DM_BF_REC;
+                    const float4 q0 = orc[0], q3 = orc[3], q4 = orc[4], q5 = orc[5];
+                    const float4 kk = skr[jz];
+                    const float kz = kk.z;
+                    const float p = fmaf(kz, q3.z, fmaf(kx, q3.x, ky * q3.y));
+                    const float q = fmaf(kz, q4.z, fmaf(kx, q4.x, ky * q4.y));
+                    const bool series = fmaxf(fmaxf(fabsf(p), fabsf(q)), fabsf(q - p)) < DM_SERIES_RADIUS;
+                    cf psi = {0.f, 0.f}, dp = {0.f, 0.f}, dq = {0.f, 0.f};
+                    if (__any_sync(0xffffffffu, have && series)) {
+                        cf a, b, c;
+                        dm_psi_series<true>(series ? p : 0.f, series ? q : 0.f, a, b, c);
+                        if (series) { psi = a; dp = b; dq = c; }
+                    }
+                    if (__any_sync(0xffffffffu, have && !series)) {
+                        cf a, b, c;
+                        dm_psi_far_uniform(series ? 0.f : p, series ? 1.f : q, a, b, c);
+                        if (!series) { psi = a; dp = b; dq = c; }
+                    }
+                    const cf E = dm_expmi_turns_fast(dm_phase_turns(nx, ny, jz, __float_as_uint(q0.x), __float_as_uint(q0.y),
+                                                                    __float_as_uint(q0.z)));
+                    const cf kE = cmul(cf{kk.x, kk.y}, E);
+                    const cf kg = cmul(kE, psi);
+                    DmBfRow v = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+                    if (have)
+                        dm_bf_add<MODE>(v, kz, fmaf(kz, q5.z, fmaf(kx, q5.x, ky * q5.y)), kg.re, kg.im,
+                                        kE.re * dp.re - kE.im * dp.im, kE.re * dq.re - kE.im * dq.im);
+                    float vv[8] = {v.S0, v.S0z, v.SI, v.SIz, v.SB, v.SBz, v.SC, v.SCz};
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int ko = __shfl_up_sync(0xffffffffu, ol, o);
+                        const bool take = lane >= o && ko == ol;
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            if (MODE == 1 && i == 1) continue;  // S0z is a volume-mode sum
+                            const float x = __shfl_up_sync(0xffffffffu, vv[i], o);
+                            if (take) vv[i] += x;
+                        }
+                    }
+                    const int kn = __shfl_down_sync(0xffffffffu, ol, 1);
+                    if (have && (lane == 31 || kn != ol)) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            if (MODE == 1 && i == 1) continue;
+                            wacc[(wrp * 8 + i) * 32 + ol] += vv[i];
+                        }
+                    }
+                    __syncwarp();
+                }
+                // owners take their sums back (and clear them)
+                if (cnt != 0) {
+                    float* a = wacc + wrp * 8 * 32 + lane;
+                    rs.S0 += a[0];
+                    if (MODE == 0) rs.S0z += a[32];
+                    rs.SI += a[64];
+                    rs.SIz += a[96];
+                    rs.SB += a[128];
+                    rs.SBz += a[160];
+                    rs.SC += a[192];
+                    rs.SCz += a[224];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) a[32 * i] = 0.f;
+                }
+                __syncwarp();
+            }
+        }
+        // fold the row into the 13 sums
+        if (MODE == 1) {
+            acc[0] += rs.S0;
+        } else {
+            acc[1] = fmaf(kx, rs.S0, acc[1]);
+            acc[2] = fmaf(ky, rs.S0, acc[2]);
+            acc[3] += rs.S0z;
+        }
+        acc[4] = fmaf(kx, rs.SI, acc[4]);
+        acc[5] = fmaf(ky, rs.SI, acc[5]);
+        acc[6] += rs.SIz;
+        acc[7] = fmaf(kx, rs.SB, acc[7]);
+        acc[8] = fmaf(ky, rs.SB, acc[8]);
+        acc[9] += rs.SBz;
+        acc[10] = fmaf(kx, rs.SC, acc[10]);
+        acc[11] = fmaf(ky, rs.SC, acc[11]);
+        acc[12] += rs.SCz;
+        __syncthreads();  // next row's buffer is complete; this row's buffer may be overwritten
+    }
+    if (live) {
+#pragma unroll
+        for (int s = 0; s < DM_BWD_NSUM; ++s) part[((size_t)blockIdx.y * DM_BWD_NSUM + s) * n_faces + t] = acc[s];
+    }
+}

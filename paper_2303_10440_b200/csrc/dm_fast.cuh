@@ -120,13 +120,6 @@ __device__ __forceinline__ float dm_gap_product(float dp, float dn, float& df)
     return __fmul_rn(__fmul_rn(dp, dn), df);
 }
 
-// fast e^{-2 pi i t} from integer turns: MUFU sin/cos on an argument reduced to [-pi, pi)
-__device__ __forceinline__ cf dm_expmi_turns_fast(uint32_t turns)
-{
-    const float x = (float)(int32_t)turns * (6.283185307179586f / 4294967296.0f);
-    return {__cosf(x), -__sinf(x)};
-}
-
 // ---- A3/A4 forward, fast kernel ---------------------------------------------------------------------------------
 // grid = (k-blocks of DM_FAST_THREADS threads, n_chunks).  part[chunk][k] receives this chunk's partial sum, already
 // multiplied by the volume-mode prefactor i/|k|^2.

@@ -132,6 +132,67 @@ __device__ __forceinline__ void dm_psi_series(float p, float q, cf& psi, cf& dp,
     }
 }
 
+// ---- branch-free ("pooled") variant of the far-pair branch -------------------------------------------------------------
+// Used for the flagged pairs of the fast backward kernel, where the 32 lanes of a warp hold UNRELATED pairs: every lane
+// runs the same instructions (roles are chosen by selects, sinc by select between polynomial and MUFU quotient), and the
+// sines / cosines are MUFU approximations on arguments reduced to [-pi, pi] (abs. error ~5e-7; these pairs are a few per
+// cent of all pairs and need ~1e-5).  Requires max gap >= DM_SERIES_RADIUS.
+__device__ __forceinline__ float dm_rcp_approx(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ void dm_sinc_dsinc_uniform(float h, float& s, float& ds)
+{
+    const float h2 = h * h;
+    const float sp = fmaf(h2, fmaf(h2, fmaf(h2, fmaf(h2, fmaf(h2, -1.0f / 39916800.0f, 1.0f / 362880.0f), -1.0f / 5040.0f),
+                                            1.0f / 120.0f), -1.0f / 6.0f), 1.0f);
+    const float dsp = h * fmaf(h2, fmaf(h2, fmaf(h2, fmaf(h2, -1.0f / 3991680.0f, 1.0f / 45360.0f), -1.0f / 840.0f),
+                                        1.0f / 30.0f), -1.0f / 3.0f);
+    const float hr = fmaf(-6.283185307179586f, rintf(h * 0.15915494309189535f), h);
+    const float sn = __sinf(hr), cs = __cosf(hr);
+    const float ih = dm_rcp_approx(h);
+    const float sb = sn * ih, dsb = (cs - sb) * ih;
+    const bool small = fabsf(h) < 0.5f;
+    s = small ? sp : sb;
+    ds = small ? dsp : dsb;
+}
+__device__ __forceinline__ void dm_dd2_uniform(float al, float be, cf& D, cf& dDa, cf& dDb)
+{
+    const float m = 0.5f * (al + be), h = 0.5f * (al - be);
+    float s, ds;
+    dm_sinc_dsinc_uniform(h, s, ds);
+    const float mr = fmaf(-6.283185307179586f, rintf(m * 0.15915494309189535f), m);
+    const cf e = {__cosf(mr), -__sinf(mr)};
+    D = cscale(e, s);
+    dDa = cmul(e, cf{0.5f * ds, -0.5f * s});
+    dDb = cmul(e, cf{-0.5f * ds, -0.5f * s});
+}
+// psi(p,q), dpsi/dp, dpsi/dq on nodes (0, p, q) with max gap >= DM_SERIES_RADIUS; same formulas as dm_psi_far
+__device__ __forceinline__ void dm_psi_far_uniform(float p, float q, cf& psi, cf& dp, cf& dq)
+{
+    const float ap = fabsf(p), aq = fabsf(q), ar = fabsf(q - p);
+    const bool A = (aq >= ap && aq >= ar);   // pair (0,2): i=0, j=1, k=2
+    const bool B = !A && (ap >= ar);         // pair (0,1): i=0, j=2, k=1;  else pair (1,2): i=1, j=0, k=2
+    const float xi = (A || B) ? 0.0f : p;
+    const float xj = A ? p : (B ? q : 0.0f);
+    const float xk = B ? p : q;
+    const float invd = dm_rcp_approx(xi - xk);
+    cf D1, D1a, D1b, D2, D2a, D2b;
+    dm_dd2_uniform(xi, xj, D1, D1a, D1b);
+    dm_dd2_uniform(xj, xk, D2, D2a, D2b);
+    psi = cscale(cmul_i(csub(D1, D2)), invd);
+    const cf dj = cscale(cmul_i(csub(D1b, D2a)), invd);
+    const cf di = cscale(csub(cmul_i(D1a), psi), invd);
+    const cf dk = cscale(csub(psi, cmul_i(D2b)), invd);
+    // node 1 is j (A), k (B) or i (C); node 2 is k (A), j (B) or k (C)
+    dp.re = A ? dj.re : (B ? dk.re : di.re);
+    dp.im = A ? dj.im : (B ? dk.im : di.im);
+    dq.re = B ? dj.re : dk.re;
+    dq.im = B ? dj.im : dk.im;
+}
+
 // psi(p,q) and its partials, any (p,q).  Robust ("slow") path.
 template <bool GRAD>
 __device__ __forceinline__ void dm_psi_robust(float p, float q, cf& psi, cf& dp, cf& dq)
@@ -163,6 +224,12 @@ __device__ __forceinline__ void dm_psi_robust(float p, float q, cf& psi, cf& dp,
 __device__ __forceinline__ uint32_t dm_phase_turns(int nx, int ny, int nz, uint32_t ux, uint32_t uy, uint32_t uz)
 {
     return (uint32_t)nx * ux + (uint32_t)ny * uy + (uint32_t)nz * uz;
+}
+// fast e^{-2 pi i t} from integer turns: MUFU sin/cos on an argument reduced exactly to [-pi, pi)
+__device__ __forceinline__ cf dm_expmi_turns_fast(uint32_t turns)
+{
+    const float x = (float)(int32_t)turns * (6.283185307179586f / 4294967296.0f);
+    return {__cosf(x), -__sinf(x)};
 }
 __device__ __forceinline__ cf dm_expmi_turns(uint32_t turns)
 {
