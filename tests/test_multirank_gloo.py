@@ -1,0 +1,92 @@
+"""World-size-2 (and 3) CPU tests of the sharded path's host logic over gloo.
+
+The CUDA kernels cannot run here, so each rank's slab reduction is computed by the oracle restricted to the rank's rows
+(tests may call the oracle); what is under test is the slab partition and the one collective of the sharded backward:
+the all-reduced partial gradients must equal the whole-grid gradient, and the slabs of F must tile the whole spectrum.
+"""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2303_10440_b200.sharding import allreduce_vertex_gradient, slab_bounds
+
+
+def test_slab_bounds_tile_the_grid():
+    for n_x in (1, 2, 5, 32, 128, 205):
+        for world in (1, 2, 3, 4, 8, 7, 300):
+            rows = []
+            for r in range(world):
+                b, e = slab_bounds(n_x, world, r)
+                assert 0 <= b <= e <= n_x
+                rows.extend(range(b, e))
+            assert rows == list(range(n_x))
+            sizes = [slab_bounds(n_x, world, r)[1] - slab_bounds(n_x, world, r)[0] for r in range(world)]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        slab_bounds(8, 2, 2)
+    with pytest.raises(ValueError):
+        slab_bounds(0, 2, 0)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out_dir):
+    import oracle
+    from workloads import build_workload
+    from workloads.configs import spectrum_cotangent
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        w = build_workload(1, grid_override=(8, 8, 8))        # 320 triangles, 8x8x5 stored frequencies
+        nx, ny, nz = w.n
+        nzh = nz // 2 + 1
+        G = spectrum_cotangent(w).astype(np.complex128)
+        b, e = slab_bounds(nx, world, rank)
+        idx = np.arange(b * ny * nzh, e * ny * nzh, dtype=np.int64)
+        for mode in (0, 1):
+            part = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, mode, G.reshape(-1)[idx],
+                                                flat_indices=idx) if len(idx) else np.zeros_like(w.vertices, dtype=np.float64)
+            dv = torch.as_tensor(np.asarray(part, dtype=np.float64))
+            allreduce_vertex_gradient(dv)
+            Fslab = oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, mode, flat_indices=idx)
+            # all-gather of the slabs of F (needed only when one rank runs the inverse FFT)
+            Fs = torch.zeros(nx * ny * nzh, dtype=torch.complex128)
+            Fs[idx] = torch.as_tensor(Fslab)
+            Fr = torch.view_as_real(Fs).clone()
+            dist.all_reduce(Fr)
+            np.save(os.path.join(out_dir, f"dv_{mode}_{rank}.npy"), dv.numpy())
+            np.save(os.path.join(out_dir, f"F_{mode}_{rank}.npy"), torch.view_as_complex(Fr).numpy())
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_sharded_backward_allreduce_matches_whole_grid(world, tmp_path):
+    import oracle
+    from workloads import build_workload
+    from workloads.configs import spectrum_cotangent
+
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    w = build_workload(1, grid_override=(8, 8, 8))
+    G = spectrum_cotangent(w).astype(np.complex128)
+    for mode in (0, 1):
+        ref = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, mode, G)
+        Fref = oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, mode).reshape(-1)
+        for r in range(world):
+            dv = np.load(tmp_path / f"dv_{mode}_{r}.npy")
+            assert np.linalg.norm(dv - ref) <= 1e-12 * np.linalg.norm(ref)
+            F = np.load(tmp_path / f"F_{mode}_{r}.npy")
+            assert np.abs(F - Fref).max() <= 1e-12 * abs(Fref[0])
