@@ -44,7 +44,7 @@ struct dm_plan {
     unsigned int* hmax2 = nullptr;   // longest squared edge (float bits), rebuilt every call
     double* dc_part = nullptr;       // [DM_DC_BLOCKS] block sums of the k = 0 entry
     int fwd_path = 0, bwd_path = 0;  // 0 = fast, 1 = robust
-    float tau = 1e-2f, tau_b = 2e-3f;
+    float tau = 1e-2f, tau_b = 2e-4f;
     cufftHandle fft_xy = 0, fft_z = 0, fft_r2c = 0;
     bool have_xy = false, have_z = false, have_r2c = false, have_fft = false;
     // stage timing
@@ -212,18 +212,31 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     int rps = 1;
     const int n_split = backward_splits(p, &rps);
     dim3 grid((p->n_faces + 127) / 128, n_split);
-    const size_t row_smem = 2 * (size_t)p->gd.nzh * sizeof(float4);
+    // seed spacing of the fast kernel: the smallest SEG whose seed table (ceil(nzh/SEG)-1 entries x 3 vertices x 128
+    // threads x 8 B) has at most 8 entries per vertex
+    const int nzh = p->gd.nzh;
+    const int seg = nzh <= 72 ? 8 : (nzh <= 144 ? 16 : 32);
+    const int n_seed = (nzh + seg - 1) / seg - 1;
+    const size_t row_smem = 2 * (size_t)nzh * sizeof(float4) + (size_t)n_seed * 3 * DM_BF_THREADS * sizeof(float2);
     int rc;
-    if (p->bwd_path == 0 && row_smem <= 32 * 1024) {
+    if (p->bwd_path == 0 && nzh <= 288) {
         dm_k_bwd_geometry<<<(p->n_faces + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->gd, p->brec);
         if ((rc = check_launch(p))) return rc;
         static_assert(DM_BF_THREADS == 128, "grid.x above assumes 128 triangles per CTA");
-        if (p->mode == DM_SURFACE)
-            dm_k_backward_fast<1><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(p->brec, p->n_faces, p->gd, p->ix_begin, p->ix_end,
-                                                                                rps, p->tau_b, (const float2*)G_dev, p->part);
-        else
-            dm_k_backward_fast<0><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(p->brec, p->n_faces, p->gd, p->ix_begin, p->ix_end,
-                                                                                rps, p->tau_b, (const float2*)G_dev, p->part);
+#define DM_LAUNCH_BF(MODE, SEG)                                                                                          \
+    do {                                                                                                                 \
+        if (cudaFuncSetAttribute(dm_k_backward_fast<MODE, SEG>, cudaFuncAttributeMaxDynamicSharedMemorySize,             \
+                                 (int)row_smem) != cudaSuccess)                                                          \
+            return DM_ERR_CUDA;                                                                                          \
+        dm_k_backward_fast<MODE, SEG><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(                                     \
+            p->brec, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, p->tau_b, (const float2*)G_dev, p->part);           \
+    } while (0)
+        if (p->mode == DM_SURFACE) {
+            if (seg == 8) DM_LAUNCH_BF(1, 8); else if (seg == 16) DM_LAUNCH_BF(1, 16); else DM_LAUNCH_BF(1, 32);
+        } else {
+            if (seg == 8) DM_LAUNCH_BF(0, 8); else if (seg == 16) DM_LAUNCH_BF(0, 16); else DM_LAUNCH_BF(0, 32);
+        }
+#undef DM_LAUNCH_BF
     } else {
         if ((rc = run_geometry(p, vertices_dev))) return rc;
         dm_k_backward_robust<<<grid, 128, 0, p->stream>>>(p->rec, p->n_faces, p->gd, p->mode, p->ix_begin, p->ix_end, rps,

@@ -17,7 +17,8 @@
 //     s0 = Re(kappa g) = sum c_j Re A_j,  sI = Im(kappa g) = sum c_j Im A_j,
 //     sb = Re(kappa dg/dx_1) = sum al_j Re A_j + c_1 Im A_1,   sc likewise.
 // Phases advance along z by one complex rotation per vertex (rotor e^{-i kstep_z v_z} built in fp64 by the geometry
-// pre-pass) and are re-seeded EXACTLY (32-bit integer turns) every DM_BF_SEG frequencies.
+// pre-pass) and are re-seeded every SEG (8, 16 or 32) frequencies from exact values: the exact row phase (32-bit
+// integer turns) times a row-independent table of exact z-phases kept in shared memory.
 //
 // Near-degenerate pairs (reading R4).  The derivative coefficients grow like 1/(gap^2 gap'), so a pair
 // with  min|gap| * |pqr| < tau_b  is excluded from the fast sums (its reciprocal is forced to 0) and flagged in a per-
@@ -30,7 +31,7 @@
 #include "dm_kernels.cuh"
 
 #define DM_BF_THREADS 128
-#define DM_BF_SEG 32            // frequencies between exact phase re-seeds = bits of the flag mask
+#define DM_BF_SEG 32            // bits of one flag word
 #define DM_BF_REC 7             // float4 per backward triangle record
 
 // backward triangle record (7 x float4 = 112 B), rebuilt every call (row A1):
@@ -80,7 +81,8 @@ __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int3
 // shared-memory queue of one warp's flagged pairs of one chunk (processed DM_BF_QCAP at a time)
 #define DM_BF_CHUNK 96          // frequencies per chunk = 3 flag words per thread
 struct DmBfQueue {
-    unsigned short code[32 * DM_BF_CHUNK];  // owner lane << 7 | frequency index inside the chunk, sorted
+    unsigned char code[32 * DM_BF_CHUNK];  // frequency index inside the chunk, in (owner lane, frequency) order; the
+                                           // owner of entry e is found from the lanes' prefix sums
 };
 
 struct dm_bf_true { static constexpr bool value = true; };
@@ -108,28 +110,73 @@ __device__ __forceinline__ void dm_bf_add(DmBfRow& a, float kz, float om, float 
     a.SCz = fmaf(kz, sc, a.SCz);
 }
 
+// The fast evaluation of ONE pair (generic closed form); returns true when the pair is excluded (flagged) instead.
+template <int MODE>
+__device__ __forceinline__ bool dm_bf_pair(const float4 kk, const float prow, const float qrow, const float omrow,
+                                           const float ebz, const float ecz, const float mz, const float tau_b,
+                                           cf& E0, cf& E1, cf& E2, const cf rho0, const cf rho1, const cf rho2, DmBfRow& rs)
+{
+    const float kz = kk.z;
+    const float p = fmaf(kz, ebz, prow), q = fmaf(kz, ecz, qrow), r = q - p;
+    const float pqr = (p * q) * r;
+    const float m1 = fminf(fminf(fabsf(p), fabsf(q)), fabsf(r));
+    const bool bad = m1 * fabsf(pqr) < tau_b;
+    const float R = bad ? 0.f : dm_rcp_approx(pqr);
+    const float c0 = -r * R, c1 = q * R, c2 = -p * R;
+    const float c0s = c0 * c0, c1s = c1 * c1, c2s = c2 * c2;
+    const float a0 = q * c0s, a2 = -q * c2s;      // al_1 = -al_0 - al_2
+    const float b0 = p * c0s, nb1 = p * c1s;      // be_1 = -nb1, be_2 = -be_0 - be_1
+    const cf kap = {kk.x, kk.y};
+    const cf A0 = cmul(kap, E0), A1 = cmul(kap, E1), A2 = cmul(kap, E2);
+#ifndef DM_BF_NODIFF
+    // every coefficient triple sums to zero, so the sums are taken on DIFFERENCES of the A_j
+    const float d01r = A0.re - A1.re, d21r = A2.re - A1.re, d02r = d01r - d21r;
+    const float d01i = A0.im - A1.im, d21i = A2.im - A1.im;
+    const float s0 = fmaf(c0, d01r, c2 * d21r);
+    const float sI = fmaf(c0, d01i, c2 * d21i);
+    const float sb = fmaf(a0, d01r, fmaf(a2, d21r, c1 * A1.im));
+    const float sc = fmaf(b0, d02r, fmaf(nb1, d21r, c2 * A2.im));
+#else
+    const float a1 = -(a0 + a2), b1 = -nb1, b2 = -(b0 + b1);
+    const float s0 = fmaf(c0, A0.re, fmaf(c1, A1.re, c2 * A2.re));
+    const float sI = fmaf(c0, A0.im, fmaf(c1, A1.im, c2 * A2.im));
+    const float sb = fmaf(a0, A0.re, fmaf(a1, A1.re, fmaf(a2, A2.re, c1 * A1.im)));
+    const float sc = fmaf(b0, A0.re, fmaf(b1, A1.re, fmaf(b2, A2.re, c2 * A2.im)));
+#endif
+    dm_bf_add<MODE>(rs, kz, fmaf(kz, mz, omrow), s0, sI, sb, sc);
+    E0 = cmul(E0, rho0);
+    E1 = cmul(E1, rho1);
+    E2 = cmul(E2, rho2);
+    return bad;
+}
+
 // ---- A6 backward, fast kernel -----------------------------------------------------------------------------------
 // grid = (ceil(n_faces / DM_BF_THREADS), n_split); part[(split*13 + s)*n_faces + t] as in dm_k_backward_robust.
-// dynamic shared memory: 2 * nzh float4 (kappa.re, kappa.im, k_z, -) double-buffered rows.
-template <int MODE>
+// SEG = frequencies between exact phase seeds (8, 16 or 32; chosen by the host so that the seed table fits).
+// dynamic shared memory: 2 * nzh float4 (kappa.re, kappa.im, k_z, -) double-buffered rows, then the seed table
+//   ztab[(a-1)*3 + j][DM_BF_THREADS] = e^{-2 pi i (a SEG) u_jz},  a = 1 .. ceil(nzh/SEG)-1, j = vertex 0..2:
+// the phase of vertex j at (row, z = a SEG) is the exact row phase e^{-2 pi i (n_x u_x + n_y u_y)} (integer turns, one
+// accurate sincospi per row) times ztab -- so a phase is never more than SEG-1 fp32 rotations away from an exact value.
+template <int MODE, int SEG>
 __global__ void __launch_bounds__(DM_BF_THREADS, 4)
 dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, int ix_begin, int ix_end,
                    int rows_per_split, float tau_b, const float2* __restrict__ G, float* __restrict__ part)
 {
+    static_assert(SEG == 8 || SEG == 16 || SEG == 32, "SEG divides the 32-bit flag word");
     extern __shared__ float4 dm_bf_smem[];
     __shared__ DmBfQueue queue[DM_BF_THREADS / 32];
-    __shared__ float4 trec[DM_BF_THREADS * DM_BF_REC];   // this CTA's triangle records (the pooled path reads other lanes')
+    __shared__ float4 trec[DM_BF_THREADS * 4];   // what the pooled path reads of other lanes' records: r0, r3, r4, r5
     __shared__ float wacc[(DM_BF_THREADS / 32) * 8 * 32];  // per warp: 8 row sums x 32 owners, filled by the pooled path
-    float4* const sk = dm_bf_smem;
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
     const int t = blockIdx.x * DM_BF_THREADS + tid;
     const bool live = t < n_faces;
     const int tt = live ? t : n_faces - 1;
-#pragma unroll
-    for (int i = 0; i < DM_BF_REC; ++i) trec[tid * DM_BF_REC + i] = rec[(size_t)DM_BF_REC * tt + i];
-    const float4 r0 = trec[tid * DM_BF_REC + 0], r1 = trec[tid * DM_BF_REC + 1], r2 = trec[tid * DM_BF_REC + 2],
-                 r3 = trec[tid * DM_BF_REC + 3], r4 = trec[tid * DM_BF_REC + 4], r5 = trec[tid * DM_BF_REC + 5],
-                 r6 = trec[tid * DM_BF_REC + 6];
+    const float4* const myrec = rec + (size_t)DM_BF_REC * tt;
+    const float4 r0 = myrec[0], r1 = myrec[1], r2 = myrec[2], r3 = myrec[3], r4 = myrec[4], r5 = myrec[5], r6 = myrec[6];
+    trec[tid * 4 + 0] = r0;
+    trec[tid * 4 + 1] = r3;
+    trec[tid * 4 + 2] = r4;
+    trec[tid * 4 + 3] = r5;
     const uint32_t u0x = __float_as_uint(r0.x), u0y = __float_as_uint(r0.y), u0z = __float_as_uint(r0.z);
     const uint32_t u1x = __float_as_uint(r1.x), u1y = __float_as_uint(r1.y), u1z = __float_as_uint(r1.z);
     const uint32_t u2x = __float_as_uint(r2.x), u2y = __float_as_uint(r2.y), u2z = __float_as_uint(r2.z);
@@ -139,7 +186,19 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
     const int row_begin = blockIdx.y * rows_per_split;
     const int row_end = min(n_rows, row_begin + rows_per_split);
     DmBfQueue& Q = queue[wrp];
-    const float4* const wrec = trec + wrp * 32 * DM_BF_REC;   // records of this warp's 32 triangles
+    const float4* const wrec = trec + wrp * 32 * 4;   // records of this warp's 32 triangles
+
+    // seed table (row-independent): exact z-phases of this thread's three vertices at every multiple of SEG
+    float4* const sk = dm_bf_smem;
+    float2* const ztab = reinterpret_cast<float2*>(dm_bf_smem + 2 * nzh);
+    const int nseg = (nzh + SEG - 1) / SEG;
+    for (int a = 1; a < nseg; ++a) {
+        const uint32_t za = (uint32_t)(a * SEG);
+        const cf z0 = dm_expmi_turns(za * u0z), z1 = dm_expmi_turns(za * u1z), z2 = dm_expmi_turns(za * u2z);
+        ztab[((a - 1) * 3 + 0) * DM_BF_THREADS + tid] = make_float2(z0.re, z0.im);
+        ztab[((a - 1) * 3 + 1) * DM_BF_THREADS + tid] = make_float2(z1.re, z1.im);
+        ztab[((a - 1) * 3 + 2) * DM_BF_THREADS + tid] = make_float2(z2.re, z2.im);
+    }
 
 #pragma unroll
     for (int i = 0; i < 8; ++i) wacc[i * DM_BF_THREADS + tid] = 0.f;
@@ -180,49 +239,54 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
         const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
         const float prow = fmaf(kx, r3.x, ky * r3.y), qrow = fmaf(kx, r4.x, ky * r4.y);
         const float omrow = fmaf(kx, r5.x, ky * r5.y);
-        const uint32_t tr0 = (uint32_t)nx * u0x + (uint32_t)ny * u0y, tr1 = (uint32_t)nx * u1x + (uint32_t)ny * u1y,
-                       tr2 = (uint32_t)nx * u2x + (uint32_t)ny * u2y;
+        // exact row phases e^{-i (k_x v_x + k_y v_y)} of the three vertices
+        const cf X0 = dm_expmi_turns((uint32_t)nx * u0x + (uint32_t)ny * u0y),
+                 X1 = dm_expmi_turns((uint32_t)nx * u1x + (uint32_t)ny * u1y),
+                 X2 = dm_expmi_turns((uint32_t)nx * u2x + (uint32_t)ny * u2y);
         DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
         for (int zc = 0; zc < nzh; zc += DM_BF_CHUNK) {
             const int clen = min(DM_BF_CHUNK, nzh - zc);
-            uint32_t fl[DM_BF_CHUNK / DM_BF_SEG];
-            // ---- fast pass over the chunk, one exactly seeded segment at a time --------------------------------------
+            uint32_t fl[DM_BF_CHUNK / 32];
+            // ---- fast pass over the chunk, one exactly seeded segment of SEG frequencies at a time ---------------------
 #pragma unroll
-            for (int sg = 0; sg < DM_BF_CHUNK / DM_BF_SEG; ++sg) {
-                fl[sg] = 0;
-                const int z0 = zc + sg * DM_BF_SEG;
-                const int len = min(DM_BF_SEG, zc + clen - z0);
-                if (len <= 0) continue;
-                cf E0 = dm_expmi_turns(tr0 + (uint32_t)z0 * u0z), E1 = dm_expmi_turns(tr1 + (uint32_t)z0 * u1z),
-                   E2 = dm_expmi_turns(tr2 + (uint32_t)z0 * u2z);
-                uint32_t flags = 0;
-#pragma unroll 4
-                for (int j = 0; j < len; ++j) {
-                    const float4 kk = skr[z0 + j];
-                    const float kz = kk.z;
-                    const float p = fmaf(kz, r3.z, prow), q = fmaf(kz, r4.z, qrow), r = q - p;
-                    const float pqr = (p * q) * r;
-                    const float m1 = fminf(fminf(fabsf(p), fabsf(q)), fabsf(r));
-                    const bool bad = m1 * fabsf(pqr) < tau_b;
-                    flags |= (bad ? 1u : 0u) << j;
-                    const float R = bad ? 0.f : dm_rcp_approx(pqr);
-                    const float c0 = -r * R, c1 = q * R, c2 = -p * R;
-                    const float c0s = c0 * c0, c1s = c1 * c1, c2s = c2 * c2;
-                    const float a0 = q * c0s, a2 = -q * c2s, a1 = -(a0 + a2);
-                    const float b0 = p * c0s, b1 = -p * c1s, b2 = -(b0 + b1);
-                    const cf kap = {kk.x, kk.y};
-                    const cf A0 = cmul(kap, E0), A1 = cmul(kap, E1), A2 = cmul(kap, E2);
-                    const float s0 = fmaf(c0, A0.re, fmaf(c1, A1.re, c2 * A2.re));
-                    const float sI = fmaf(c0, A0.im, fmaf(c1, A1.im, c2 * A2.im));
-                    const float sb = fmaf(a0, A0.re, fmaf(a1, A1.re, fmaf(a2, A2.re, c1 * A1.im)));
-                    const float sc = fmaf(b0, A0.re, fmaf(b1, A1.re, fmaf(b2, A2.re, c2 * A2.im)));
-                    dm_bf_add<MODE>(rs, kz, fmaf(kz, r5.z, omrow), s0, sI, sb, sc);
-                    E0 = cmul(E0, rho0);
-                    E1 = cmul(E1, rho1);
-                    E2 = cmul(E2, rho2);
+            for (int w = 0; w < DM_BF_CHUNK / 32; ++w) {
+                uint32_t word = 0;
+                const int wbeg = zc + 32 * w;
+                const int wlen = min(32, zc + clen - wbeg);
+                if (wlen > 0) {
+                    const int nfull = wlen / SEG;
+                    int z0 = wbeg;
+#pragma unroll 1
+                    for (int s = 0; s <= nfull; ++s, z0 += SEG) {
+                        const int len = (s < nfull) ? SEG : wlen - nfull * SEG;
+                        if (len == 0) break;
+                        cf E0 = X0, E1 = X1, E2 = X2;
+                        if (z0 > 0) {
+                            const float2* zt = ztab + (size_t)(z0 / SEG - 1) * 3 * DM_BF_THREADS + tid;
+                            const float2 a0 = zt[0], a1 = zt[DM_BF_THREADS], a2 = zt[2 * DM_BF_THREADS];
+                            E0 = cmul(X0, cf{a0.x, a0.y});
+                            E1 = cmul(X1, cf{a1.x, a1.y});
+                            E2 = cmul(X2, cf{a2.x, a2.y});
+                        }
+                        uint32_t sf = 0;
+                        if (len == SEG) {
+#pragma unroll
+                            for (int j = 0; j < SEG; ++j)
+                                if (dm_bf_pair<MODE>(skr[z0 + j], prow, qrow, omrow, r3.z, r4.z, r5.z, tau_b, E0, E1, E2, rho0,
+                                                     rho1, rho2, rs))
+                                    sf |= 1u << j;
+                        } else {
+#pragma unroll 1
+                            for (int j = 0; j < len; ++j)
+                                if (dm_bf_pair<MODE>(skr[z0 + j], prow, qrow, omrow, r3.z, r4.z, r5.z, tau_b, E0, E1, E2, rho0,
+                                                     rho1, rho2, rs))
+                                    sf |= 1u << j;
+                        }
+                        word |= sf << (s * SEG);
+                    }
                 }
-                fl[sg] = live ? flags : 0u;
+                fl[w] = live ? word : 0u;
             }
             // ---- pooled slow path -------------------------------------------------------------------------------------
             int cnt = 0;
@@ -244,7 +308,7 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
                     while (f) {
                         const int j = __ffs(f) - 1;
                         f &= f - 1;
-                        Q.code[w++] = (unsigned short)((lane << 7) | (sg * DM_BF_SEG + j));
+                        Q.code[w++] = (unsigned char)(sg * DM_BF_SEG + j);
                     }
                 }
                 __syncwarp();
@@ -253,10 +317,17 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
                 for (int base = 0; base < total; base += 32) {
                     const int e = base + lane;
                     const bool have = e < total;
-                    const int code = have ? Q.code[e] : 0;
-                    const int ol = have ? (code >> 7) : -1 - lane, jz = zc + (code & 127);
-                    const float4* orc = wrec + (code >> 7) * DM_BF_REC;
-                    const float4 q0 = orc[0], q3 = orc[3], q4 = orc[4], q5 = orc[5];
+                    // owner of entry e = number of lanes whose inclusive prefix sum is <= e (binary search by shuffles)
+                    int own = 0;
+#pragma unroll
+                    for (int st = 16; st > 0; st >>= 1) {
+                        const int v = __shfl_sync(0xffffffffu, off, own + st - 1);
+                        if (v <= e) own += st;
+                    }
+                    own = have ? own : 0;
+                    const int ol = have ? own : -1 - lane, jz = zc + (have ? (int)Q.code[e] : 0);
+                    const float4* orc = wrec + own * 4;
+                    const float4 q0 = orc[0], q3 = orc[1], q4 = orc[2], q5 = orc[3];
                     const float4 kk = skr[jz];
                     const float kz = kk.z;
                     const float p = fmaf(kz, q3.z, fmaf(kx, q3.x, ky * q3.y));
