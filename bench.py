@@ -158,6 +158,10 @@ def run_ours(args):
     # every rank owns one mesh of the same recipe (independent problems; seed offset = rank)
     w = build_workload(args.cfg, seed_offset=rank)
     plan = dm.Plan(w.n, w.spacing, w.origin, w.mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    slab = None
+    if args.x_slab:  # profiling aid: restrict the mesh-FT calls to rows [a, b) of the stored spectrum (not a bench number)
+        slab = tuple(int(x) for x in args.x_slab.split(":"))
+        plan.set_slab(*slab)
     vd = torch.as_tensor(w.vertices, device="cuda")
     Gd = torch.as_tensor(spectrum_cotangent(w), device="cuda")
     F = torch.empty(w.spectrum_shape, dtype=torch.complex64, device="cuda")
@@ -203,7 +207,12 @@ def run_ours(args):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     step_ms, fwd_ms, bwd_ms = (float(x) for x in t.tolist())
-    pairs = float(w.pairs)
+    pairs = float(w.pairs) if slab is None else float(w.faces.shape[0]) * (slab[1] - slab[0]) * w.n[1] * (w.n[2] // 2 + 1)
+    if slab is not None:
+        if rank == 0:
+            print(json.dumps({"profiling_only": True, "x_slab": list(slab), "pairs": pairs, "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
+                              "bwd_kernel_ms": float(np.mean(bwd_kernel_ms))}), flush=True)
+        return
 
     # ---- end to end through the public API with HOST buffers (render + render_backward) ---------------------------
     hv = torch.as_tensor(w.vertices).pin_memory()
@@ -302,6 +311,8 @@ def main():
     ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json config 1..5 (default 4, the target config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-freqs", type=int, default=192, help="stored frequencies per oracle sample")
+    ap.add_argument("--x-slab", default="", help="a:b -- profiling aid (ncu counters overflow on the 0.4 s full-grid launch): run "
+                    "forward/backward on rows [a,b) of the spectrum only and print a short line that is NOT a bench result")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

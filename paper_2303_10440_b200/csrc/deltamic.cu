@@ -215,7 +215,11 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     // seed spacing of the fast kernel: the smallest SEG whose seed table (ceil(nzh/SEG)-1 entries x 3 vertices x 128
     // threads x 8 B) has at most 8 entries per vertex
     const int nzh = p->gd.nzh;
+#if defined(DM_BF_FORCE_SEG)
+    const int seg = DM_BF_FORCE_SEG;
+#else
     const int seg = nzh <= 72 ? 8 : (nzh <= 144 ? 16 : 32);
+#endif
     const int n_seed = (nzh + seg - 1) / seg - 1;
     const size_t row_smem = 2 * (size_t)nzh * sizeof(float4) + (size_t)n_seed * 3 * DM_BF_THREADS * sizeof(float2);
     int rc;

@@ -32,6 +32,7 @@
 
 #define DM_BF_THREADS 128
 #define DM_BF_SEG 32            // bits of one flag word
+#define DM_BF_UNR 8             // unroll of the fast loop
 #define DM_BF_REC 7             // float4 per backward triangle record
 
 // backward triangle record (7 x float4 = 112 B), rebuilt every call (row A1):
@@ -249,30 +250,34 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
             const int clen = min(DM_BF_CHUNK, nzh - zc);
             uint32_t fl[DM_BF_CHUNK / 32];
             // ---- fast pass over the chunk, one exactly seeded segment of SEG frequencies at a time ---------------------
+            // (the body is unrolled by DM_BF_UNR whatever SEG is: longer bodies fall out of the instruction cache)
+            cf E0 = X0, E1 = X1, E2 = X2;
 #pragma unroll
             for (int w = 0; w < DM_BF_CHUNK / 32; ++w) {
                 uint32_t word = 0;
                 const int wbeg = zc + 32 * w;
                 const int wlen = min(32, zc + clen - wbeg);
                 if (wlen > 0) {
-                    const int nfull = wlen / SEG;
+                    const int nfull = wlen / DM_BF_UNR;
                     int z0 = wbeg;
 #pragma unroll 1
-                    for (int s = 0; s <= nfull; ++s, z0 += SEG) {
-                        const int len = (s < nfull) ? SEG : wlen - nfull * SEG;
+                    for (int s = 0; s <= nfull; ++s, z0 += DM_BF_UNR) {
+                        const int len = (s < nfull) ? DM_BF_UNR : wlen - nfull * DM_BF_UNR;
                         if (len == 0) break;
-                        cf E0 = X0, E1 = X1, E2 = X2;
-                        if (z0 > 0) {
-                            const float2* zt = ztab + (size_t)(z0 / SEG - 1) * 3 * DM_BF_THREADS + tid;
-                            const float2 a0 = zt[0], a1 = zt[DM_BF_THREADS], a2 = zt[2 * DM_BF_THREADS];
-                            E0 = cmul(X0, cf{a0.x, a0.y});
-                            E1 = cmul(X1, cf{a1.x, a1.y});
-                            E2 = cmul(X2, cf{a2.x, a2.y});
+                        if ((z0 & (SEG - 1)) == 0) {   // exact seed
+                            E0 = X0, E1 = X1, E2 = X2;
+                            if (z0 > 0) {
+                                const float2* zt = ztab + (size_t)(z0 / SEG - 1) * 3 * DM_BF_THREADS + tid;
+                                const float2 a0 = zt[0], a1 = zt[DM_BF_THREADS], a2 = zt[2 * DM_BF_THREADS];
+                                E0 = cmul(X0, cf{a0.x, a0.y});
+                                E1 = cmul(X1, cf{a1.x, a1.y});
+                                E2 = cmul(X2, cf{a2.x, a2.y});
+                            }
                         }
                         uint32_t sf = 0;
-                        if (len == SEG) {
+                        if (len == DM_BF_UNR) {
 #pragma unroll
-                            for (int j = 0; j < SEG; ++j)
+                            for (int j = 0; j < DM_BF_UNR; ++j)
                                 if (dm_bf_pair<MODE>(skr[z0 + j], prow, qrow, omrow, r3.z, r4.z, r5.z, tau_b, E0, E1, E2, rho0,
                                                      rho1, rho2, rs))
                                     sf |= 1u << j;
@@ -283,7 +288,7 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
                                                      rho1, rho2, rs))
                                     sf |= 1u << j;
                         }
-                        word |= sf << (s * SEG);
+                        word |= sf << (s * DM_BF_UNR);
                     }
                 }
                 fl[w] = live ? word : 0u;
