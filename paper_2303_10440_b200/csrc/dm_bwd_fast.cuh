@@ -1,10 +1,18 @@
 // dm_bwd_fast.cuh -- optimised backward mesh-FT kernel (rows A1, A6 of the hot path), sm_100a.
 //
-// Layout.  One THREAD owns one triangle and keeps its 13 k-sums in registers; a CTA of DM_BF_THREADS triangles walks a
-// range of (i_x,i_y) rows of the stored spectrum, innermost along z.  Every thread of the CTA is at the SAME frequency
-// at the same time, so everything that depends on k only -- kappa = conj(G) (surface) or i conj(G)/|k|^2 (volume), k_z --
-// is computed once per CTA and row into shared memory and read back as one broadcast LDS.128 per pair: there is no
-// reduction across threads at all (O(N n_v) backward; :182-186 eq. 13 is the later CSR gather).
+// Layout.  One THREAD owns one triangle and keeps its 13 k-sums in registers; one WARP owns a compact patch of 32
+// triangles (dm_patches.h) and a CTA of four warps walks a range of (i_x,i_y) rows of the stored spectrum, innermost
+// along z.  Every thread of the CTA is at the SAME frequency at the same time, so everything that depends on k only --
+// kappa = conj(G) (surface) or i conj(G)/|k|^2 (volume), k_z -- is computed once per CTA and row into shared memory and
+// read back as one broadcast LDS.128 per pair, and there is no reduction across threads at all (O(N n_v)
+// backward; :182-186 eq. 13 is the later CSR gather).
+//
+// Shared vertex phases (north_star: "each vertex's phase e^{-ik.v} is computed once per (k-tile, vertex) and reused across
+// its incident triangles").  A patch of 32 triangles has about 28 distinct vertices.  Lane l owns vertex slot l of its
+// patch (and slot 32+l in the few patches with more than 32 vertices): per frequency it advances that ONE phase by a
+// complex rotation, multiplies it by kappa and stores A_v = kappa e^{-ik.v} in shared memory; after a __syncwarp the 32
+// triangle lanes read the A_v of their three corners.  Per pair this is 8 FP32 operations + 1 STS + 3 LDS instead of the
+// 24 operations of three private phases.
 //
 // Arithmetic of the generic pair.  With nodes x_j = k.v_j, E_j = e^{-i x_j} and gaps
 // p = x_1-x_0, q = x_2-x_0, r = q-p, eq. 9 is  g = sum_j c_j E_j  with REAL coefficients
@@ -15,10 +23,11 @@
 //     dg/dx_0 = -i g - dg/dx_1 - dg/dx_2.
 // With A_j = kappa E_j the four real numbers a pair contributes are
 //     s0 = Re(kappa g) = sum c_j Re A_j,  sI = Im(kappa g) = sum c_j Im A_j,
-//     sb = Re(kappa dg/dx_1) = sum al_j Re A_j + c_1 Im A_1,   sc likewise.
-// Phases advance along z by one complex rotation per vertex (rotor e^{-i kstep_z v_z} built in fp64 by the geometry
-// pre-pass) and are re-seeded every SEG (8, 16 or 32) frequencies from exact values: the exact row phase (32-bit
-// integer turns) times a row-independent table of exact z-phases kept in shared memory.
+//     sb = Re(kappa dg/dx_1) = sum al_j Re A_j + c_1 Im A_1,   sc likewise,
+// all taken on differences of the A_j (every coefficient triple sums to zero).
+// Phases advance along z by one complex rotation (rotor e^{-i kstep_z v_z} built in fp64 by the geometry pre-pass) and
+// are re-seeded every SEG (8, 16 or 32) frequencies from exact values: the exact row phase (32-bit integer turns) times a
+// row-independent table of exact z-phases kept in shared memory.
 //
 // Near-degenerate pairs (reading R4).  The derivative coefficients grow like 1/(gap^2 gap'), so a pair
 // with  min|gap| * |pqr| < tau_b  is excluded from the fast sums (its reciprocal is forced to 0) and flagged in a per-
@@ -29,65 +38,94 @@
 // reproducible (reading R22), and the divergent work is spread evenly over the lanes.
 #pragma once
 #include "dm_kernels.cuh"
+#include "dm_patches.h"
 
 #define DM_BF_THREADS 128
 #define DM_BF_SEG 32            // bits of one flag word
 #define DM_BF_UNR 8             // unroll of the fast loop
-#define DM_BF_REC 7             // float4 per backward triangle record
+#ifndef DM_BF_STAGE
+#define DM_BF_STAGE 4           // frequencies whose vertex phases are staged in shared memory at a time (divides DM_BF_UNR)
+#endif
+#define DM_BF_TREC 4            // float4 per triangle record
+#define DM_BF_VREC 2            // float4 per vertex-slot record
 
-// backward triangle record (7 x float4 = 112 B), rebuilt every call (row A1):
-//   r0..r2 = (u_j.xyz [uint32 bit patterns: v_j / L in fixed-point turns], -)   j = 0,1,2
-//   r3 = (eb.xyz, rho_0.re)   r4 = (ec.xyz, rho_0.im)   r5 = (m_T.xyz, |m_T|)   r6 = (rho_1.re, rho_1.im, rho_2.re, rho_2.im)
-//   eb = v_1-v_0, ec = v_2-v_0, rho_j = e^{-i kstep_z v_jz}
-__global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int32_t* __restrict__ faces, int n_faces,
-                                  DmGridDev grid, float4* __restrict__ rec)
+// device copies of the patch tables (topology; built at plan creation)
+struct DmPatchDev {
+    const int32_t* face;    // [n_lanes]       face of lane, -1 = idle
+    const int32_t* vid;     // [n_lanes * 2]   vertex of slot s of patch P at [P*64 + s], -1 = unused
+    const uint32_t* loc;    // [n_lanes]       corner slots l0 | l1 << 8 | l2 << 16
+    const int32_t* nv;      // [n_lanes / 32]  1 or 2 vertex slots per lane
+    int n_lanes;            // 32 * number of patches, a multiple of DM_BF_THREADS
+};
+
+// Records rebuilt every call (row A1), indexed by lane i = 32 * patch + l:
+//   triangle  trec[4i..4i+3] = (u_0.xyz [uint32 bit patterns: v_0 / L in fixed-point turns], loc bits)
+//                              (eb.xyz, -)   (ec.xyz, -)   (m_T.xyz, |m_T|)       eb = v_1-v_0, ec = v_2-v_0
+//   vertex    vrec[2s..2s+1], s = 64 * patch + slot:  (u.xyz turns, rho.re)  (rho.im, -, -, -),  rho = e^{-i kstep_z v_z}
+__global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int32_t* __restrict__ faces, DmPatchDev pt,
+                                  DmGridDev grid, float4* __restrict__ trec, float4* __restrict__ vrec)
 {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= n_faces) return;
-    float v[3][3];
-    uint32_t u[3][3];
-    float rho[3][2];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= pt.n_lanes) return;
+    {
+        int f = pt.face[i];
+        if (f < 0) f = pt.face[i & ~31];   // idle lane: any valid triangle of the patch (lane 0 holds one)
+        if (f < 0) f = 0;                  // padding patch
+        float v[3][3];
 #pragma unroll
-    for (int j = 0; j < 3; ++j) {
-        const int i = faces[3 * t + j];
+        for (int j = 0; j < 3; ++j) {
+            const int iv = faces[3 * f + j];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) v[j][d] = vertices[3 * iv + d];
+        }
+        uint32_t u[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            v[j][d] = vertices[3 * i + d];
-            double tt = (double)v[j][d] * grid.inv_len[d];
+            double tt = (double)v[0][d] * grid.inv_len[d];
             tt -= floor(tt);
-            u[j][d] = (uint32_t)(unsigned long long)(tt * 4294967296.0 + 0.5);
+            u[d] = (uint32_t)(unsigned long long)(tt * 4294967296.0 + 0.5);
         }
-        double tz = (double)v[j][2] * grid.inv_len[2];
-        tz -= rint(tz);
-        double sn, cs;
-        sincospi(2.0 * tz, &sn, &cs);
-        rho[j][0] = (float)cs;
-        rho[j][1] = (float)(-sn);
+        const float eb[3] = {v[1][0] - v[0][0], v[1][1] - v[0][1], v[1][2] - v[0][2]};
+        const float ec[3] = {v[2][0] - v[0][0], v[2][1] - v[0][1], v[2][2] - v[0][2]};
+        const float m[3] = {eb[1] * ec[2] - eb[2] * ec[1], eb[2] * ec[0] - eb[0] * ec[2], eb[0] * ec[1] - eb[1] * ec[0]};
+        const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+        float4* o = trec + (size_t)DM_BF_TREC * i;
+        o[0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), __uint_as_float(pt.loc[i]));
+        o[1] = make_float4(eb[0], eb[1], eb[2], 0.f);
+        o[2] = make_float4(ec[0], ec[1], ec[2], 0.f);
+        o[3] = make_float4(m[0], m[1], m[2], mn);
     }
-    const float eb[3] = {v[1][0] - v[0][0], v[1][1] - v[0][1], v[1][2] - v[0][2]};
-    const float ec[3] = {v[2][0] - v[0][0], v[2][1] - v[0][1], v[2][2] - v[0][2]};
-    const float m[3] = {eb[1] * ec[2] - eb[2] * ec[1], eb[2] * ec[0] - eb[0] * ec[2], eb[0] * ec[1] - eb[1] * ec[0]};
-    const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
-    float4* o = rec + (size_t)DM_BF_REC * t;
 #pragma unroll
-    for (int j = 0; j < 3; ++j)
-        o[j] = make_float4(__uint_as_float(u[j][0]), __uint_as_float(u[j][1]), __uint_as_float(u[j][2]), 0.f);
-    o[3] = make_float4(eb[0], eb[1], eb[2], rho[0][0]);
-    o[4] = make_float4(ec[0], ec[1], ec[2], rho[0][1]);
-    o[5] = make_float4(m[0], m[1], m[2], mn);
-    o[6] = make_float4(rho[1][0], rho[1][1], rho[2][0], rho[2][1]);
+    for (int h = 0; h < 2; ++h) {
+        const size_t s = (size_t)(i >> 5) * DM_PATCH_MAXV + 32 * h + (i & 31);
+        const int iv = pt.vid[s];
+        float4 a = make_float4(0.f, 0.f, 0.f, 1.f), b = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (iv >= 0) {
+            uint32_t u[3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                double tt = (double)vertices[3 * iv + d] * grid.inv_len[d];
+                tt -= floor(tt);
+                u[d] = (uint32_t)(unsigned long long)(tt * 4294967296.0 + 0.5);
+            }
+            double tz = (double)vertices[3 * iv + 2] * grid.inv_len[2];
+            tz -= rint(tz);
+            double sn, cs;
+            sincospi(2.0 * tz, &sn, &cs);
+            a = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), (float)cs);
+            b.x = (float)(-sn);
+        }
+        vrec[DM_BF_VREC * s] = a;
+        vrec[DM_BF_VREC * s + 1] = b;
+    }
 }
 
-
-// shared-memory queue of one warp's flagged pairs of one chunk (processed DM_BF_QCAP at a time)
+// shared-memory queue of one warp's flagged pairs of one chunk
 #define DM_BF_CHUNK 96          // frequencies per chunk = 3 flag words per thread
 struct DmBfQueue {
     unsigned char code[32 * DM_BF_CHUNK];  // frequency index inside the chunk, in (owner lane, frequency) order; the
                                            // owner of entry e is found from the lanes' prefix sums
 };
-
-struct dm_bf_true { static constexpr bool value = true; };
-struct dm_bf_false { static constexpr bool value = false; };
 
 // what one pair adds to the row sums (plain and k_z-weighted sums of s0, sI, sb, sc)
 struct DmBfRow {
@@ -111,13 +149,13 @@ __device__ __forceinline__ void dm_bf_add(DmBfRow& a, float kz, float om, float 
     a.SCz = fmaf(kz, sc, a.SCz);
 }
 
-// The fast evaluation of ONE pair (generic closed form); returns true when the pair is excluded (flagged) instead.
+// The fast evaluation of ONE pair (generic closed form) from the staged A_j = kappa e^{-i x_j} of its three corners;
+// returns true when the pair is excluded (flagged) instead.
 template <int MODE>
-__device__ __forceinline__ bool dm_bf_pair(const float4 kk, const float prow, const float qrow, const float omrow,
-                                           const float ebz, const float ecz, const float mz, const float tau_b,
-                                           cf& E0, cf& E1, cf& E2, const cf rho0, const cf rho1, const cf rho2, DmBfRow& rs)
+__device__ __forceinline__ bool dm_bf_pair(const float kz, const cf A0, const cf A1, const cf A2, const float prow,
+                                           const float qrow, const float omrow, const float ebz, const float ecz,
+                                           const float mz, const float tau_b, DmBfRow& rs)
 {
-    const float kz = kk.z;
     const float p = fmaf(kz, ebz, prow), q = fmaf(kz, ecz, qrow), r = q - p;
     const float pqr = (p * q) * r;
     const float m1 = fminf(fminf(fabsf(p), fabsf(q)), fabsf(r));
@@ -127,78 +165,76 @@ __device__ __forceinline__ bool dm_bf_pair(const float4 kk, const float prow, co
     const float c0s = c0 * c0, c1s = c1 * c1, c2s = c2 * c2;
     const float a0 = q * c0s, a2 = -q * c2s;      // al_1 = -al_0 - al_2
     const float b0 = p * c0s, nb1 = p * c1s;      // be_1 = -nb1, be_2 = -be_0 - be_1
-    const cf kap = {kk.x, kk.y};
-    const cf A0 = cmul(kap, E0), A1 = cmul(kap, E1), A2 = cmul(kap, E2);
-#ifndef DM_BF_NODIFF
-    // every coefficient triple sums to zero, so the sums are taken on DIFFERENCES of the A_j
     const float d01r = A0.re - A1.re, d21r = A2.re - A1.re, d02r = d01r - d21r;
     const float d01i = A0.im - A1.im, d21i = A2.im - A1.im;
     const float s0 = fmaf(c0, d01r, c2 * d21r);
     const float sI = fmaf(c0, d01i, c2 * d21i);
     const float sb = fmaf(a0, d01r, fmaf(a2, d21r, c1 * A1.im));
     const float sc = fmaf(b0, d02r, fmaf(nb1, d21r, c2 * A2.im));
-#else
-    const float a1 = -(a0 + a2), b1 = -nb1, b2 = -(b0 + b1);
-    const float s0 = fmaf(c0, A0.re, fmaf(c1, A1.re, c2 * A2.re));
-    const float sI = fmaf(c0, A0.im, fmaf(c1, A1.im, c2 * A2.im));
-    const float sb = fmaf(a0, A0.re, fmaf(a1, A1.re, fmaf(a2, A2.re, c1 * A1.im)));
-    const float sc = fmaf(b0, A0.re, fmaf(b1, A1.re, fmaf(b2, A2.re, c2 * A2.im)));
-#endif
     dm_bf_add<MODE>(rs, kz, fmaf(kz, mz, omrow), s0, sI, sb, sc);
-    E0 = cmul(E0, rho0);
-    E1 = cmul(E1, rho1);
-    E2 = cmul(E2, rho2);
     return bad;
 }
 
 // ---- A6 backward, fast kernel -----------------------------------------------------------------------------------
-// grid = (ceil(n_faces / DM_BF_THREADS), n_split); part[(split*13 + s)*n_faces + t] as in dm_k_backward_robust.
-// SEG = frequencies between exact phase seeds (8, 16 or 32; chosen by the host so that the seed table fits).
-// dynamic shared memory: 2 * nzh float4 (kappa.re, kappa.im, k_z, -) double-buffered rows, then the seed table
-//   ztab[(a-1)*3 + j][DM_BF_THREADS] = e^{-2 pi i (a SEG) u_jz},  a = 1 .. ceil(nzh/SEG)-1, j = vertex 0..2:
-// the phase of vertex j at (row, z = a SEG) is the exact row phase e^{-2 pi i (n_x u_x + n_y u_y)} (integer turns, one
-// accurate sincospi per row) times ztab -- so a phase is never more than SEG-1 fp32 rotations away from an exact value.
+// grid = (n_lanes / DM_BF_THREADS, n_split): one warp per patch; part[(split*13 + s)*n_faces + face] as in
+// dm_k_backward_robust.  SEG = frequencies between exact phase seeds (8, 16 or 32; chosen by the host so that the seed
+// table fits).  Dynamic shared memory:
+//   2 * nzh float4                      double-buffered rows (kappa.re, kappa.im, k_z, -)
+//   (nseg-1) * 2 * 128 float2           seed table ztab[(a-1)*2 + h][tid] = e^{-2 pi i (a SEG) u_z} of the thread's vertex
+//                                       slot h, a = 1 .. nseg-1, nseg = ceil(nzh/SEG): with the exact row phase
+//                                       e^{-2 pi i (n_x u_x + n_y u_y)} (integer turns, one accurate sincospi per row) a
+//                                       phase is never more than SEG-1 fp32 rotations away from an exact value
+//   4 * DM_BF_STAGE * 64 float2         per warp: A_v = kappa e^{-ik.v} of the patch's vertex slots for DM_BF_STAGE
+//                                       consecutive frequencies
 template <int MODE, int SEG>
 __global__ void __launch_bounds__(DM_BF_THREADS, 4)
-dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, int ix_begin, int ix_end,
-                   int rows_per_split, float tau_b, const float2* __restrict__ G, float* __restrict__ part)
+dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__ vrec_g, DmPatchDev pt, int n_faces,
+                   DmGridDev grid, int ix_begin, int ix_end, int rows_per_split, float tau_b,
+                   const float2* __restrict__ G, float* __restrict__ part)
 {
     static_assert(SEG == 8 || SEG == 16 || SEG == 32, "SEG divides the 32-bit flag word");
+    static_assert(DM_BF_UNR % DM_BF_STAGE == 0 && SEG % DM_BF_UNR == 0, "stages tile the unrolled body, bodies tile a segment");
     extern __shared__ float4 dm_bf_smem[];
     __shared__ DmBfQueue queue[DM_BF_THREADS / 32];
-    __shared__ float4 trec[DM_BF_THREADS * 4];   // what the pooled path reads of other lanes' records: r0, r3, r4, r5
+    __shared__ float4 trec[DM_BF_THREADS * DM_BF_TREC];    // this CTA's triangle records (the pooled path reads other lanes')
     __shared__ float wacc[(DM_BF_THREADS / 32) * 8 * 32];  // per warp: 8 row sums x 32 owners, filled by the pooled path
+    float4* const sk = dm_bf_smem;
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
-    const int t = blockIdx.x * DM_BF_THREADS + tid;
-    const bool live = t < n_faces;
-    const int tt = live ? t : n_faces - 1;
-    const float4* const myrec = rec + (size_t)DM_BF_REC * tt;
-    const float4 r0 = myrec[0], r1 = myrec[1], r2 = myrec[2], r3 = myrec[3], r4 = myrec[4], r5 = myrec[5], r6 = myrec[6];
-    trec[tid * 4 + 0] = r0;
-    trec[tid * 4 + 1] = r3;
-    trec[tid * 4 + 2] = r4;
-    trec[tid * 4 + 3] = r5;
-    const uint32_t u0x = __float_as_uint(r0.x), u0y = __float_as_uint(r0.y), u0z = __float_as_uint(r0.z);
-    const uint32_t u1x = __float_as_uint(r1.x), u1y = __float_as_uint(r1.y), u1z = __float_as_uint(r1.z);
-    const uint32_t u2x = __float_as_uint(r2.x), u2y = __float_as_uint(r2.y), u2z = __float_as_uint(r2.z);
-    const cf rho0 = {r3.w, r4.w}, rho1 = {r6.x, r6.y}, rho2 = {r6.z, r6.w};
+    const int gl = blockIdx.x * DM_BF_THREADS + tid;       // global lane = 32 * patch + lane
+    const int face = pt.face[gl];
+    const bool live = face >= 0;
+    const float4 r0 = trec_g[(size_t)DM_BF_TREC * gl], r3 = trec_g[(size_t)DM_BF_TREC * gl + 1],
+                 r4 = trec_g[(size_t)DM_BF_TREC * gl + 2], r5 = trec_g[(size_t)DM_BF_TREC * gl + 3];
+    trec[tid * DM_BF_TREC + 0] = r0;
+    trec[tid * DM_BF_TREC + 1] = r3;
+    trec[tid * DM_BF_TREC + 2] = r4;
+    trec[tid * DM_BF_TREC + 3] = r5;
+    const uint32_t loc = __float_as_uint(r0.w);
+    const int l0 = (int)(loc & 255u), l1 = (int)((loc >> 8) & 255u), l2 = (int)((loc >> 16) & 255u);
+    const bool two = pt.nv[gl >> 5] > 1;                   // warp-uniform: the patch has more than 32 vertices
+    // the vertex slots this lane owns: slot lane (a) and slot 32 + lane (b)
+    const size_t vs = (size_t)(gl >> 5) * DM_PATCH_MAXV + lane;
+    const float4 va0 = vrec_g[DM_BF_VREC * vs], va1 = vrec_g[DM_BF_VREC * vs + 1];
+    const float4 vb0 = vrec_g[DM_BF_VREC * (vs + 32)], vb1 = vrec_g[DM_BF_VREC * (vs + 32) + 1];
+    const uint32_t uax = __float_as_uint(va0.x), uay = __float_as_uint(va0.y), uaz = __float_as_uint(va0.z);
+    const uint32_t ubx = __float_as_uint(vb0.x), uby = __float_as_uint(vb0.y), ubz = __float_as_uint(vb0.z);
+    const cf rhoa = {va0.w, va1.x}, rhob = {vb0.w, vb1.x};
     const int nzh = grid.nzh;
     const int n_rows = (ix_end - ix_begin) * grid.ny;
     const int row_begin = blockIdx.y * rows_per_split;
     const int row_end = min(n_rows, row_begin + rows_per_split);
     DmBfQueue& Q = queue[wrp];
-    const float4* const wrec = trec + wrp * 32 * 4;   // records of this warp's 32 triangles
+    const float4* const wrec = trec + wrp * 32 * DM_BF_TREC;   // records of this warp's 32 triangles
 
-    // seed table (row-independent): exact z-phases of this thread's three vertices at every multiple of SEG
-    float4* const sk = dm_bf_smem;
-    float2* const ztab = reinterpret_cast<float2*>(dm_bf_smem + 2 * nzh);
+    // seed table (row-independent): exact z-phases of this thread's vertex slots at every multiple of SEG
     const int nseg = (nzh + SEG - 1) / SEG;
+    float2* const ztab = reinterpret_cast<float2*>(dm_bf_smem + 2 * nzh);
+    float2* const at = ztab + (size_t)(nseg - 1) * 2 * DM_BF_THREADS + wrp * DM_BF_STAGE * DM_PATCH_MAXV;
     for (int a = 1; a < nseg; ++a) {
         const uint32_t za = (uint32_t)(a * SEG);
-        const cf z0 = dm_expmi_turns(za * u0z), z1 = dm_expmi_turns(za * u1z), z2 = dm_expmi_turns(za * u2z);
-        ztab[((a - 1) * 3 + 0) * DM_BF_THREADS + tid] = make_float2(z0.re, z0.im);
-        ztab[((a - 1) * 3 + 1) * DM_BF_THREADS + tid] = make_float2(z1.re, z1.im);
-        ztab[((a - 1) * 3 + 2) * DM_BF_THREADS + tid] = make_float2(z2.re, z2.im);
+        const cf z0 = dm_expmi_turns(za * uaz), z1 = dm_expmi_turns(za * ubz);
+        ztab[((a - 1) * 2 + 0) * DM_BF_THREADS + tid] = make_float2(z0.re, z0.im);
+        ztab[((a - 1) * 2 + 1) * DM_BF_THREADS + tid] = make_float2(z1.re, z1.im);
     }
 
 #pragma unroll
@@ -229,6 +265,63 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
         }
     };
 
+    // one stage of n <= DM_BF_STAGE frequencies starting at z: every lane writes A_v of its vertex slot(s), then every
+    // lane evaluates its triangle at those frequencies; returns the flags of the stage (bit j = frequency z + j)
+    auto run_stage = [&](const float4* skr, int z, int n, bool full, cf& Ea, cf& Eb, float prow, float qrow, float omrow,
+                         DmBfRow& rs) -> uint32_t {
+        if (full) {
+#pragma unroll
+            for (int j = 0; j < DM_BF_STAGE; ++j) {
+                const float4 kk = skr[z + j];
+                const cf A = cmul(cf{kk.x, kk.y}, Ea);
+                at[j * DM_PATCH_MAXV + lane] = make_float2(A.re, A.im);
+                Ea = cmul(Ea, rhoa);
+            }
+            if (two) {
+#pragma unroll
+                for (int j = 0; j < DM_BF_STAGE; ++j) {
+                    const float4 kk = skr[z + j];
+                    const cf A = cmul(cf{kk.x, kk.y}, Eb);
+                    at[j * DM_PATCH_MAXV + 32 + lane] = make_float2(A.re, A.im);
+                    Eb = cmul(Eb, rhob);
+                }
+            }
+        } else {
+#pragma unroll 1
+            for (int j = 0; j < n; ++j) {
+                const float4 kk = skr[z + j];
+                const cf A = cmul(cf{kk.x, kk.y}, Ea), B = cmul(cf{kk.x, kk.y}, Eb);
+                at[j * DM_PATCH_MAXV + lane] = make_float2(A.re, A.im);
+                at[j * DM_PATCH_MAXV + 32 + lane] = make_float2(B.re, B.im);
+                Ea = cmul(Ea, rhoa);
+                Eb = cmul(Eb, rhob);
+            }
+        }
+        __syncwarp();
+        uint32_t sf = 0;
+        if (full) {
+#pragma unroll
+            for (int j = 0; j < DM_BF_STAGE; ++j) {
+                const float kz = skr[z + j].z;
+                const float2 a0 = at[j * DM_PATCH_MAXV + l0], a1 = at[j * DM_PATCH_MAXV + l1], a2 = at[j * DM_PATCH_MAXV + l2];
+                if (dm_bf_pair<MODE>(kz, cf{a0.x, a0.y}, cf{a1.x, a1.y}, cf{a2.x, a2.y}, prow, qrow, omrow, r3.z, r4.z, r5.z,
+                                     tau_b, rs))
+                    sf |= 1u << j;
+            }
+        } else {
+#pragma unroll 1
+            for (int j = 0; j < n; ++j) {
+                const float kz = skr[z + j].z;
+                const float2 a0 = at[j * DM_PATCH_MAXV + l0], a1 = at[j * DM_PATCH_MAXV + l1], a2 = at[j * DM_PATCH_MAXV + l2];
+                if (dm_bf_pair<MODE>(kz, cf{a0.x, a0.y}, cf{a1.x, a1.y}, cf{a2.x, a2.y}, prow, qrow, omrow, r3.z, r4.z, r5.z,
+                                     tau_b, rs))
+                    sf |= 1u << j;
+            }
+        }
+        __syncwarp();
+        return sf;
+    };
+
     if (row_begin < row_end) stage_row(row_begin, 0);
     __syncthreads();
     for (int row = row_begin; row < row_end; ++row) {
@@ -240,18 +333,17 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
         const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
         const float prow = fmaf(kx, r3.x, ky * r3.y), qrow = fmaf(kx, r4.x, ky * r4.y);
         const float omrow = fmaf(kx, r5.x, ky * r5.y);
-        // exact row phases e^{-i (k_x v_x + k_y v_y)} of the three vertices
-        const cf X0 = dm_expmi_turns((uint32_t)nx * u0x + (uint32_t)ny * u0y),
-                 X1 = dm_expmi_turns((uint32_t)nx * u1x + (uint32_t)ny * u1y),
-                 X2 = dm_expmi_turns((uint32_t)nx * u2x + (uint32_t)ny * u2y);
+        // exact row phases e^{-i (k_x v_x + k_y v_y)} of the lane's vertex slots
+        const cf Xa = dm_expmi_turns((uint32_t)nx * uax + (uint32_t)ny * uay);
+        cf Xb = {1.f, 0.f};
+        if (two) Xb = dm_expmi_turns((uint32_t)nx * ubx + (uint32_t)ny * uby);
         DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
         for (int zc = 0; zc < nzh; zc += DM_BF_CHUNK) {
             const int clen = min(DM_BF_CHUNK, nzh - zc);
             uint32_t fl[DM_BF_CHUNK / 32];
-            // ---- fast pass over the chunk, one exactly seeded segment of SEG frequencies at a time ---------------------
-            // (the body is unrolled by DM_BF_UNR whatever SEG is: longer bodies fall out of the instruction cache)
-            cf E0 = X0, E1 = X1, E2 = X2;
+            // ---- fast pass over the chunk: bodies of DM_BF_UNR frequencies, exact seeds every SEG ---------------------
+            cf Ea = Xa, Eb = Xb;
 #pragma unroll
             for (int w = 0; w < DM_BF_CHUNK / 32; ++w) {
                 uint32_t word = 0;
@@ -265,28 +357,24 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
                         const int len = (s < nfull) ? DM_BF_UNR : wlen - nfull * DM_BF_UNR;
                         if (len == 0) break;
                         if ((z0 & (SEG - 1)) == 0) {   // exact seed
-                            E0 = X0, E1 = X1, E2 = X2;
+                            Ea = Xa, Eb = Xb;
                             if (z0 > 0) {
-                                const float2* zt = ztab + (size_t)(z0 / SEG - 1) * 3 * DM_BF_THREADS + tid;
-                                const float2 a0 = zt[0], a1 = zt[DM_BF_THREADS], a2 = zt[2 * DM_BF_THREADS];
-                                E0 = cmul(X0, cf{a0.x, a0.y});
-                                E1 = cmul(X1, cf{a1.x, a1.y});
-                                E2 = cmul(X2, cf{a2.x, a2.y});
+                                const float2* zt = ztab + (size_t)(z0 / SEG - 1) * 2 * DM_BF_THREADS + tid;
+                                const float2 a0 = zt[0], a1 = zt[DM_BF_THREADS];
+                                Ea = cmul(Xa, cf{a0.x, a0.y});
+                                Eb = cmul(Xb, cf{a1.x, a1.y});
                             }
                         }
                         uint32_t sf = 0;
                         if (len == DM_BF_UNR) {
 #pragma unroll
-                            for (int j = 0; j < DM_BF_UNR; ++j)
-                                if (dm_bf_pair<MODE>(skr[z0 + j], prow, qrow, omrow, r3.z, r4.z, r5.z, tau_b, E0, E1, E2, rho0,
-                                                     rho1, rho2, rs))
-                                    sf |= 1u << j;
+                            for (int h = 0; h < DM_BF_UNR / DM_BF_STAGE; ++h)
+                                sf |= run_stage(skr, z0 + h * DM_BF_STAGE, DM_BF_STAGE, true, Ea, Eb, prow, qrow, omrow, rs)
+                                      << (h * DM_BF_STAGE);
                         } else {
 #pragma unroll 1
-                            for (int j = 0; j < len; ++j)
-                                if (dm_bf_pair<MODE>(skr[z0 + j], prow, qrow, omrow, r3.z, r4.z, r5.z, tau_b, E0, E1, E2, rho0,
-                                                     rho1, rho2, rs))
-                                    sf |= 1u << j;
+                            for (int j0 = 0; j0 < len; j0 += DM_BF_STAGE)
+                                sf |= run_stage(skr, z0 + j0, min(DM_BF_STAGE, len - j0), false, Ea, Eb, prow, qrow, omrow, rs) << j0;
                         }
                         word |= sf << (s * DM_BF_UNR);
                     }
@@ -417,6 +505,6 @@ dm_k_backward_fast(const float4* __restrict__ rec, int n_faces, DmGridDev grid, 
     }
     if (live) {
 #pragma unroll
-        for (int s = 0; s < DM_BWD_NSUM; ++s) part[((size_t)blockIdx.y * DM_BWD_NSUM + s) * n_faces + t] = acc[s];
+        for (int s = 0; s < DM_BWD_NSUM; ++s) part[((size_t)blockIdx.y * DM_BWD_NSUM + s) * n_faces + face] = acc[s];
     }
 }
