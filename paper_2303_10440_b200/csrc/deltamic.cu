@@ -31,11 +31,11 @@ struct dm_plan {
     int32_t* csr_corner = nullptr;   // [n_faces*3]   3*face+corner, ascending per vertex
     float4* rec = nullptr;           // [n_faces*4]   triangle records (A1)
     // patches of the fast backward kernel (topology only; built at create) and its per-call records
-    int32_t *pt_face = nullptr, *pt_vid = nullptr, *pt_nv = nullptr;
+    int32_t *pt_face = nullptr, *pt_vid = nullptr;
     uint32_t* pt_loc = nullptr;
     int pt_lanes = 0;                // 32 * patches, padded to a multiple of DM_BF_THREADS
     float4* btrec = nullptr;         // [pt_lanes*DM_BF_TREC] backward triangle records (A1)
-    float4* bvrec = nullptr;         // [pt_lanes*2*DM_BF_VREC] backward vertex-slot records (A1)
+    float4* bvrec = nullptr;         // [pt_lanes*DM_BF_VREC] backward vertex-slot records (A1)
     float* part = nullptr;           // [n_split_max*13*n_faces]
     float* corner = nullptr;         // [n_faces*9]
     float2* spec = nullptr;          // [n_k] scratch spectrum (S, R or G)
@@ -226,11 +226,11 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     const int seg = nzh <= 72 ? 8 : (nzh <= 144 ? 16 : 32);
 #endif
     const int n_seed = (nzh + seg - 1) / seg - 1;
-    const size_t row_smem = 2 * (size_t)nzh * sizeof(float4) + (size_t)n_seed * 2 * DM_BF_THREADS * sizeof(float2) +
+    const size_t row_smem = 2 * (size_t)nzh * sizeof(float4) + (size_t)n_seed * DM_BF_THREADS * sizeof(float2) +
                             (size_t)(DM_BF_THREADS / 32) * DM_BF_STAGE * DM_PATCH_MAXV * sizeof(float2);
     int rc;
     if (p->bwd_path == 0 && nzh <= 288) {
-        const DmPatchDev pt = {p->pt_face, p->pt_vid, p->pt_loc, p->pt_nv, p->pt_lanes};
+        const DmPatchDev pt = {p->pt_face, p->pt_vid, p->pt_loc, p->pt_lanes};
         grid.x = (unsigned)(p->pt_lanes / DM_BF_THREADS);
         dm_k_bwd_geometry<<<p->pt_lanes / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, pt, p->gd, p->btrec, p->bvrec);
         if ((rc = check_launch(p))) return rc;
@@ -425,7 +425,6 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
                     pp.face.insert(pp.face.end(), DM_PATCH_FACES, -1);
                     pp.loc.insert(pp.loc.end(), DM_PATCH_FACES, 0u);
                     pp.vid.insert(pp.vid.end(), DM_PATCH_MAXV, -1);
-                    pp.nv.push_back(1);
                 }
             } catch (...) { rc = DM_ERR_ALLOC; break; }
             p->pt_lanes = (int)pp.face.size();
@@ -433,13 +432,11 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
             if (cudaMalloc(&p->pt_face, nl * sizeof(int32_t)) != cudaSuccess ||
                 cudaMalloc(&p->pt_loc, nl * sizeof(uint32_t)) != cudaSuccess ||
                 cudaMalloc(&p->pt_vid, pp.vid.size() * sizeof(int32_t)) != cudaSuccess ||
-                cudaMalloc(&p->pt_nv, pp.nv.size() * sizeof(int32_t)) != cudaSuccess ||
                 cudaMalloc(&p->btrec, nl * DM_BF_TREC * sizeof(float4)) != cudaSuccess ||
-                cudaMalloc(&p->bvrec, nl * 2 * DM_BF_VREC * sizeof(float4)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
+                cudaMalloc(&p->bvrec, nl * DM_BF_VREC * sizeof(float4)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
             if (cudaMemcpyAsync(p->pt_face, pp.face.data(), nl * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
                 cudaMemcpyAsync(p->pt_loc, pp.loc.data(), nl * sizeof(uint32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
                 cudaMemcpyAsync(p->pt_vid, pp.vid.data(), pp.vid.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
-                cudaMemcpyAsync(p->pt_nv, pp.nv.data(), pp.nv.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
                 cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
         }
         bool ok = true;
@@ -587,7 +584,6 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->rec);
     cudaFree(p->pt_face);
     cudaFree(p->pt_vid);
-    cudaFree(p->pt_nv);
     cudaFree(p->pt_loc);
     cudaFree(p->btrec);
     cudaFree(p->bvrec);

@@ -9,7 +9,7 @@
 //
 // Shared vertex phases (north_star: "each vertex's phase e^{-ik.v} is computed once per (k-tile, vertex) and reused across
 // its incident triangles").  A patch of 32 triangles has about 28 distinct vertices.  Lane l owns vertex slot l of its
-// patch (and slot 32+l in the few patches with more than 32 vertices): per frequency it advances that ONE phase by a
+// patch: per frequency it advances that ONE phase by a
 // complex rotation, multiplies it by kappa and stores A_v = kappa e^{-ik.v} in shared memory; after a __syncwarp the 32
 // triangle lanes read the A_v of their three corners.  Per pair this is 8 FP32 operations + 1 STS + 3 LDS instead of the
 // 24 operations of three private phases.
@@ -41,6 +41,9 @@
 #include "dm_patches.h"
 
 #define DM_BF_THREADS 128
+#ifndef DM_BF_MINCTA
+#define DM_BF_MINCTA 5         // resident CTAs per SM the register allocation aims at (<= 102 registers)
+#endif
 #define DM_BF_SEG 32            // bits of one flag word
 #define DM_BF_UNR 8             // unroll of the fast loop
 #ifndef DM_BF_STAGE
@@ -52,16 +55,15 @@
 // device copies of the patch tables (topology; built at plan creation)
 struct DmPatchDev {
     const int32_t* face;    // [n_lanes]       face of lane, -1 = idle
-    const int32_t* vid;     // [n_lanes * 2]   vertex of slot s of patch P at [P*64 + s], -1 = unused
+    const int32_t* vid;     // [n_lanes]       vertex of slot l of the patch, -1 = unused
     const uint32_t* loc;    // [n_lanes]       corner slots l0 | l1 << 8 | l2 << 16
-    const int32_t* nv;      // [n_lanes / 32]  1 or 2 vertex slots per lane
     int n_lanes;            // 32 * number of patches, a multiple of DM_BF_THREADS
 };
 
 // Records rebuilt every call (row A1), indexed by lane i = 32 * patch + l:
 //   triangle  trec[4i..4i+3] = (u_0.xyz [uint32 bit patterns: v_0 / L in fixed-point turns], loc bits)
 //                              (eb.xyz, -)   (ec.xyz, -)   (m_T.xyz, |m_T|)       eb = v_1-v_0, ec = v_2-v_0
-//   vertex    vrec[2s..2s+1], s = 64 * patch + slot:  (u.xyz turns, rho.re)  (rho.im, -, -, -),  rho = e^{-i kstep_z v_z}
+//   vertex    vrec[2i..2i+1] (slot l of the patch):  (u.xyz turns, rho.re)  (rho.im, -, -, -),  rho = e^{-i kstep_z v_z}
 __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int32_t* __restrict__ faces, DmPatchDev pt,
                                   DmGridDev grid, float4* __restrict__ trec, float4* __restrict__ vrec)
 {
@@ -95,9 +97,8 @@ __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int3
         o[2] = make_float4(ec[0], ec[1], ec[2], 0.f);
         o[3] = make_float4(m[0], m[1], m[2], mn);
     }
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-        const size_t s = (size_t)(i >> 5) * DM_PATCH_MAXV + 32 * h + (i & 31);
+    {
+        const size_t s = (size_t)i;
         const int iv = pt.vid[s];
         float4 a = make_float4(0.f, 0.f, 0.f, 1.f), b = make_float4(0.f, 0.f, 0.f, 0.f);
         if (iv >= 0) {
@@ -180,14 +181,14 @@ __device__ __forceinline__ bool dm_bf_pair(const float kz, const cf A0, const cf
 // dm_k_backward_robust.  SEG = frequencies between exact phase seeds (8, 16 or 32; chosen by the host so that the seed
 // table fits).  Dynamic shared memory:
 //   2 * nzh float4                      double-buffered rows (kappa.re, kappa.im, k_z, -)
-//   (nseg-1) * 2 * 128 float2           seed table ztab[(a-1)*2 + h][tid] = e^{-2 pi i (a SEG) u_z} of the thread's vertex
-//                                       slot h, a = 1 .. nseg-1, nseg = ceil(nzh/SEG): with the exact row phase
+//   (nseg-1) * 128 float2               seed table ztab[a-1][tid] = e^{-2 pi i (a SEG) u_z} of the thread's vertex
+//                                       slot, a = 1 .. nseg-1, nseg = ceil(nzh/SEG): with the exact row phase
 //                                       e^{-2 pi i (n_x u_x + n_y u_y)} (integer turns, one accurate sincospi per row) a
 //                                       phase is never more than SEG-1 fp32 rotations away from an exact value
-//   4 * DM_BF_STAGE * 64 float2         per warp: A_v = kappa e^{-ik.v} of the patch's vertex slots for DM_BF_STAGE
+//   4 * DM_BF_STAGE * 32 float2         per warp: A_v = kappa e^{-ik.v} of the patch's vertex slots for DM_BF_STAGE
 //                                       consecutive frequencies
 template <int MODE, int SEG>
-__global__ void __launch_bounds__(DM_BF_THREADS, 4)
+__global__ void __launch_bounds__(DM_BF_THREADS, DM_BF_MINCTA)
 dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__ vrec_g, DmPatchDev pt, int n_faces,
                    DmGridDev grid, int ix_begin, int ix_end, int rows_per_split, float tau_b,
                    const float2* __restrict__ G, float* __restrict__ part)
@@ -211,14 +212,10 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
     trec[tid * DM_BF_TREC + 3] = r5;
     const uint32_t loc = __float_as_uint(r0.w);
     const int l0 = (int)(loc & 255u), l1 = (int)((loc >> 8) & 255u), l2 = (int)((loc >> 16) & 255u);
-    const bool two = pt.nv[gl >> 5] > 1;                   // warp-uniform: the patch has more than 32 vertices
-    // the vertex slots this lane owns: slot lane (a) and slot 32 + lane (b)
-    const size_t vs = (size_t)(gl >> 5) * DM_PATCH_MAXV + lane;
-    const float4 va0 = vrec_g[DM_BF_VREC * vs], va1 = vrec_g[DM_BF_VREC * vs + 1];
-    const float4 vb0 = vrec_g[DM_BF_VREC * (vs + 32)], vb1 = vrec_g[DM_BF_VREC * (vs + 32) + 1];
+    // the vertex slot this lane owns (slot lane of its patch)
+    const float4 va0 = vrec_g[(size_t)DM_BF_VREC * gl], va1 = vrec_g[(size_t)DM_BF_VREC * gl + 1];
     const uint32_t uax = __float_as_uint(va0.x), uay = __float_as_uint(va0.y), uaz = __float_as_uint(va0.z);
-    const uint32_t ubx = __float_as_uint(vb0.x), uby = __float_as_uint(vb0.y), ubz = __float_as_uint(vb0.z);
-    const cf rhoa = {va0.w, va1.x}, rhob = {vb0.w, vb1.x};
+    const cf rhoa = {va0.w, va1.x};
     const int nzh = grid.nzh;
     const int n_rows = (ix_end - ix_begin) * grid.ny;
     const int row_begin = blockIdx.y * rows_per_split;
@@ -229,12 +226,11 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
     // seed table (row-independent): exact z-phases of this thread's vertex slots at every multiple of SEG
     const int nseg = (nzh + SEG - 1) / SEG;
     float2* const ztab = reinterpret_cast<float2*>(dm_bf_smem + 2 * nzh);
-    float2* const at = ztab + (size_t)(nseg - 1) * 2 * DM_BF_THREADS + wrp * DM_BF_STAGE * DM_PATCH_MAXV;
+    float2* const at = ztab + (size_t)(nseg - 1) * DM_BF_THREADS + wrp * DM_BF_STAGE * DM_PATCH_MAXV;
     for (int a = 1; a < nseg; ++a) {
         const uint32_t za = (uint32_t)(a * SEG);
-        const cf z0 = dm_expmi_turns(za * uaz), z1 = dm_expmi_turns(za * ubz);
-        ztab[((a - 1) * 2 + 0) * DM_BF_THREADS + tid] = make_float2(z0.re, z0.im);
-        ztab[((a - 1) * 2 + 1) * DM_BF_THREADS + tid] = make_float2(z1.re, z1.im);
+        const cf z0 = dm_expmi_turns(za * uaz);
+        ztab[(a - 1) * DM_BF_THREADS + tid] = make_float2(z0.re, z0.im);
     }
 
 #pragma unroll
@@ -267,7 +263,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
 
     // one stage of n <= DM_BF_STAGE frequencies starting at z: every lane writes A_v of its vertex slot(s), then every
     // lane evaluates its triangle at those frequencies; returns the flags of the stage (bit j = frequency z + j)
-    auto run_stage = [&](const float4* skr, int z, int n, bool full, cf& Ea, cf& Eb, float prow, float qrow, float omrow,
+    auto run_stage = [&](const float4* skr, int z, int n, bool full, cf& Ea, float prow, float qrow, float omrow,
                          DmBfRow& rs) -> uint32_t {
         if (full) {
 #pragma unroll
@@ -277,24 +273,13 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
                 at[j * DM_PATCH_MAXV + lane] = make_float2(A.re, A.im);
                 Ea = cmul(Ea, rhoa);
             }
-            if (two) {
-#pragma unroll
-                for (int j = 0; j < DM_BF_STAGE; ++j) {
-                    const float4 kk = skr[z + j];
-                    const cf A = cmul(cf{kk.x, kk.y}, Eb);
-                    at[j * DM_PATCH_MAXV + 32 + lane] = make_float2(A.re, A.im);
-                    Eb = cmul(Eb, rhob);
-                }
-            }
         } else {
 #pragma unroll 1
             for (int j = 0; j < n; ++j) {
                 const float4 kk = skr[z + j];
-                const cf A = cmul(cf{kk.x, kk.y}, Ea), B = cmul(cf{kk.x, kk.y}, Eb);
+                const cf A = cmul(cf{kk.x, kk.y}, Ea);
                 at[j * DM_PATCH_MAXV + lane] = make_float2(A.re, A.im);
-                at[j * DM_PATCH_MAXV + 32 + lane] = make_float2(B.re, B.im);
                 Ea = cmul(Ea, rhoa);
-                Eb = cmul(Eb, rhob);
             }
         }
         __syncwarp();
@@ -333,17 +318,15 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
         const float prow = fmaf(kx, r3.x, ky * r3.y), qrow = fmaf(kx, r4.x, ky * r4.y);
         const float omrow = fmaf(kx, r5.x, ky * r5.y);
-        // exact row phases e^{-i (k_x v_x + k_y v_y)} of the lane's vertex slots
+        // exact row phase e^{-i (k_x v_x + k_y v_y)} of the lane's vertex slot
         const cf Xa = dm_expmi_turns((uint32_t)nx * uax + (uint32_t)ny * uay);
-        cf Xb = {1.f, 0.f};
-        if (two) Xb = dm_expmi_turns((uint32_t)nx * ubx + (uint32_t)ny * uby);
         DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
         for (int zc = 0; zc < nzh; zc += DM_BF_CHUNK) {
             const int clen = min(DM_BF_CHUNK, nzh - zc);
             uint32_t fl[DM_BF_CHUNK / 32];
             // ---- fast pass over the chunk: bodies of DM_BF_UNR frequencies, exact seeds every SEG ---------------------
-            cf Ea = Xa, Eb = Xb;
+            cf Ea = Xa;
 #pragma unroll
             for (int w = 0; w < DM_BF_CHUNK / 32; ++w) {
                 uint32_t word = 0;
@@ -357,24 +340,22 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
                         const int len = (s < nfull) ? DM_BF_UNR : wlen - nfull * DM_BF_UNR;
                         if (len == 0) break;
                         if ((z0 & (SEG - 1)) == 0) {   // exact seed
-                            Ea = Xa, Eb = Xb;
+                            Ea = Xa;
                             if (z0 > 0) {
-                                const float2* zt = ztab + (size_t)(z0 / SEG - 1) * 2 * DM_BF_THREADS + tid;
-                                const float2 a0 = zt[0], a1 = zt[DM_BF_THREADS];
+                                const float2 a0 = ztab[(size_t)(z0 / SEG - 1) * DM_BF_THREADS + tid];
                                 Ea = cmul(Xa, cf{a0.x, a0.y});
-                                Eb = cmul(Xb, cf{a1.x, a1.y});
                             }
                         }
                         uint32_t sf = 0;
                         if (len == DM_BF_UNR) {
 #pragma unroll
                             for (int h = 0; h < DM_BF_UNR / DM_BF_STAGE; ++h)
-                                sf |= run_stage(skr, z0 + h * DM_BF_STAGE, DM_BF_STAGE, true, Ea, Eb, prow, qrow, omrow, rs)
+                                sf |= run_stage(skr, z0 + h * DM_BF_STAGE, DM_BF_STAGE, true, Ea, prow, qrow, omrow, rs)
                                       << (h * DM_BF_STAGE);
                         } else {
 #pragma unroll 1
                             for (int j0 = 0; j0 < len; j0 += DM_BF_STAGE)
-                                sf |= run_stage(skr, z0 + j0, min(DM_BF_STAGE, len - j0), false, Ea, Eb, prow, qrow, omrow, rs) << j0;
+                                sf |= run_stage(skr, z0 + j0, min(DM_BF_STAGE, len - j0), false, Ea, prow, qrow, omrow, rs) << j0;
                         }
                         word |= sf << (s * DM_BF_UNR);
                     }

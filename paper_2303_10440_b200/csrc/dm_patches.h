@@ -8,8 +8,9 @@
 //
 // Patches are grown as breadth-first balls over the face adjacency: a patch starts at the first unassigned face of a
 // global breadth-first order, adds unassigned faces ring by ring until it holds 32, and -- when its ball runs out of
-// unassigned faces first -- continues from the next unassigned face, so every patch but the last holds exactly 32 faces
-// (no idle lanes).  A patch is closed early only if another face would push it past DM_PATCH_MAXV distinct vertices.
+// unassigned faces first -- continues from the next unassigned face, so almost every patch holds exactly 32 faces.  A
+// patch is closed early (its remaining lanes idle) when another face would push it past DM_PATCH_MAXV = 32 distinct
+// vertices, one per lane: a few per cent of the patches, each losing a few lanes.
 #pragma once
 #include <cstdint>
 #include <deque>
@@ -18,13 +19,12 @@
 #include "dm_strips.h"
 
 #define DM_PATCH_FACES 32
-#define DM_PATCH_MAXV 64   // vertex slots of a patch: lane l owns slots l and 32 + l
+#define DM_PATCH_MAXV 32   // vertex slots of a patch: lane l owns slot l
 
 struct DmPatches {
     std::vector<int32_t> face;   // [n_patches*32]  face id of lane l, or -1 (idle lane)
-    std::vector<int32_t> vid;    // [n_patches*64]  vertex id of slot s, or -1
+    std::vector<int32_t> vid;    // [n_patches*32]  vertex id of slot s, or -1
     std::vector<uint32_t> loc;   // [n_patches*32]  slots of the face's corners 0,1,2: l0 | l1 << 8 | l2 << 16
-    std::vector<int32_t> nv;     // [n_patches]     1 if the patch has <= 32 vertices, else 2
     int64_t n_patches = 0;
 };
 
@@ -108,7 +108,6 @@ inline DmPatches dm_build_patches(const int32_t* faces, int32_t n_f, int32_t n_v
             }
         }
         for (int s = 0; s < DM_PATCH_MAXV; ++s) out.vid.push_back(s < (int)pv.size() ? pv[s] : -1);
-        out.nv.push_back(pv.size() <= 32 ? 1 : 2);
         for (int32_t v : pv) slot_of[v] = -1;
         ++out.n_patches;
     }
