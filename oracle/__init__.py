@@ -20,4 +20,5 @@ from .mesh_ft import (  # noqa: F401
     mesh_ft_backward_grid,
     num_threads,
 )
-from .render import psf_shift_spectrum, render, render_backward, spectrum_to_image, image_to_spectrum_cotangent  # noqa: F401
+from .render import (psf_shift_spectrum, render, render_backward, render_backward_psf, spectrum_to_image,  # noqa: F401
+                     image_to_spectrum_cotangent)

@@ -64,3 +64,29 @@ def render_backward(vertices, faces, n, spacing, origin, psf_cov, mode: int, dL_
     from .mesh_ft import mesh_ft_backward_grid
     G = image_to_spectrum_cotangent(dL_dimage, n, spacing, origin, psf_cov)
     return mesh_ft_backward_grid(vertices, faces, n, spacing, mode, G)
+
+
+def render_backward_psf(vertices, faces, n, spacing, origin, psf_cov, mode: int, dL_dimage) -> np.ndarray:
+    """dL/dSigma as 6 numbers in the order of ``psf_cov`` (xx, yy, zz, xy, xz, yz), the off-diagonal entries being the
+    derivative with respect to the ONE number that fills both symmetric positions of Sigma (the
+    PSF parameters are optimised by gradient descent; eq. 4 with reading R5).
+
+    With S = F c, c = exp(-1/2 k^T Sigma k) e^{i k.x0}/(h_x h_y h_z):  dS/dSigma_aa = -1/2 k_a^2 S,
+    dS/dSigma_ab = -k_a k_b S (a != b), and dL/dS = (w/N_tot) rfftn(dL/dimage) on independent stored entries
+    (reading R14), so  dL/dSigma_m = sum_k Re( conj(dL/dS) dS/dSigma_m ).
+    """
+    from .mesh_ft import mesh_ft_forward_grid
+    n = tuple(int(v) for v in n)
+    F = mesh_ft_forward_grid(vertices, faces, n, spacing, mode)
+    S = np.asarray(F, dtype=np.complex128) * psf_shift_spectrum(n, spacing, origin, psf_cov)
+    g = np.asarray(dL_dimage, dtype=np.float64).reshape(n)
+    dS = np.fft.rfftn(g, axes=(0, 1, 2)) / float(np.prod(n))
+    w = np.full(n[2] // 2 + 1, 2.0)
+    w[0] = 1.0
+    if n[2] % 2 == 0:
+        w[-1] = 1.0
+    t = (np.conj(dS * w[None, None, :]) * S).real
+    k = frequency_grid(n, spacing)
+    kx, ky, kz = k[..., 0], k[..., 1], k[..., 2]
+    q = [-0.5 * kx * kx, -0.5 * ky * ky, -0.5 * kz * kz, -kx * ky, -kx * kz, -ky * kz]
+    return np.array([float((qm * t).sum()) for qm in q])

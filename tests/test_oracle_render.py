@@ -96,3 +96,42 @@ def test_render_backward_vs_finite_differences_through_the_whole_render():
                 fd[i, d] = ((oracle.render(vp, f, n, spacing, origin, cov, mode) * y).sum()
                             - (oracle.render(vm, f, n, spacing, origin, cov, mode) * y).sum()) / (2 * h)
         assert np.linalg.norm(grad - fd) / np.linalg.norm(fd) < 1e-7
+
+
+def test_psf_gradient_vs_finite_differences_of_the_render():
+    """NEXT 2: dL/dSigma of the oracle against central differences of its own render in each
+    of the six covariance entries, with a full (non-diagonal) covariance and an anisotropic grid."""
+    n = (8, 10, 12)
+    spacing = (1 / 8, 1 / 10, 1 / 6)
+    origin = tuple(-0.5 * nn * h + 0.5 * h for nn, h in zip(n, spacing))
+    cov = np.array([0.020, 0.028, 0.045, 0.004, -0.006, 0.009])
+    v, f = icosphere(1, 0.3, (0.02, 0.01, -0.03))
+    y = np.random.default_rng(11).standard_normal(n)
+    for mode in (0, 1):
+        grad = oracle.render_backward_psf(v, f, n, spacing, origin, cov, mode, y)
+        fd = np.zeros(6)
+        for m in range(6):
+            h = 1e-6
+            cp, cm = cov.copy(), cov.copy()
+            cp[m] += h
+            cm[m] -= h
+            fd[m] = ((oracle.render(v, f, n, spacing, origin, cp, mode) * y).sum()
+                     - (oracle.render(v, f, n, spacing, origin, cm, mode) * y).sum()) / (2 * h)
+        assert np.abs(grad - fd).max() <= 1e-7 * np.abs(fd).max(), (mode, grad, fd)
+
+
+def test_psf_gradient_of_total_intensity_is_zero_and_blur_lowers_peak():
+    """Closed-form checks: sum(image) = F(0)/voxel does not depend on Sigma (k = 0 has zero weight), so dL/dSigma = 0 for
+    L = sum(image); and for L = image at the centre voxel of a small blob more blur lowers the peak: dL/dSigma_aa < 0."""
+    n = (12, 12, 12)
+    spacing = (1 / 12,) * 3
+    origin = (-0.5 + 1 / 24,) * 3
+    cov = [(1.5 / 12) ** 2] * 3 + [0, 0, 0]
+    v, f = icosphere(1, 0.12, (1 / 24, 1 / 24, 1 / 24))
+    g = oracle.render_backward_psf(v, f, n, spacing, origin, cov, 0, np.ones(n))
+    img = oracle.render(v, f, n, spacing, origin, cov, 0)
+    assert np.abs(g).max() <= 1e-9 * np.abs(img).sum()
+    y = np.zeros(n)
+    y[6, 6, 6] = 1.0
+    g = oracle.render_backward_psf(v, f, n, spacing, origin, cov, 0, y)
+    assert (g[:3] < 0).all()
