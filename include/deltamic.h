@@ -113,8 +113,11 @@ int dm_render(dm_plan* plan, const float* vertices_dev, const float* psf_cov_hos
 /* Backward of dm_render with respect to the vertices.
  *   dL_dimage_dev      float32 [n_x*n_y*n_z]
  *   dL_dvertices_dev   float32 [n_vertices*3], overwritten
- *   dL_dpsf_cov_host   NULL, or 6 floats on the host; a non-NULL pointer returns DM_ERR_UNSUPPORTED
- *                      until the PSF-parameter gradient is built. */
+ *   dL_dpsf_cov_host   NULL, or 6 floats on the HOST that receive dL/dSigma in the order of psf_cov_host
+ *                      (the PSF parameters are fitted by gradient descent); an off-diagonal
+ *                      entry is the derivative with respect to the one number that fills both symmetric positions.
+ *                      When non-NULL the call recomputes the forward mesh FT of these vertices (one extra
+ *                      dm_mesh_ft_forward) and SYNCHRONISES the stream before it returns. */
 int dm_render_backward(dm_plan* plan, const float* vertices_dev, const float* psf_cov_host,
                        const float* dL_dimage_dev, float* dL_dvertices_dev, float* dL_dpsf_cov_host);
 

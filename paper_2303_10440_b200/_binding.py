@@ -185,15 +185,19 @@ class Plan:
         _check(self._lib.dm_render(self._h, v.data_ptr(), _cov(psf_cov), o.data_ptr()), "dm_render")
         return out
 
-    def render_backward(self, vertices, psf_cov, dL_dimage, out=None):
+    def render_backward(self, vertices, psf_cov, dL_dimage, out=None, with_psf_grad: bool = False):
+        """dL/dvertices; with ``with_psf_grad`` also dL/dSigma (6 floats, host) as a second return value."""
         torch = self._torch
         v = self._vertices(vertices)
         g = self._f32(dL_dimage, self.n[0] * self.n[1] * self.n[2], "dL_dimage")
         if out is None:
             out = torch.empty((self.n_vertices, 3), dtype=torch.float32, device=self.device)
         o = self._f32(out, self.n_vertices * 3, "dL_dvertices")
-        _check(self._lib.dm_render_backward(self._h, v.data_ptr(), _cov(psf_cov), g.data_ptr(), o.data_ptr(), None),
+        dcov = (ctypes.c_float * 6)() if with_psf_grad else None
+        _check(self._lib.dm_render_backward(self._h, v.data_ptr(), _cov(psf_cov), g.data_ptr(), o.data_ptr(), dcov),
                "dm_render_backward")
+        if with_psf_grad:
+            return out, [float(x) for x in dcov]
         return out
 
     def spectrum_to_image(self, F, psf_cov, out=None):

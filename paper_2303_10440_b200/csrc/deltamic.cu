@@ -48,6 +48,9 @@ struct dm_plan {
     float2* fwd_part = nullptr;      // [st_n_chunks * n_k] per-chunk partial spectra
     unsigned int* hmax2 = nullptr;   // longest squared edge (float bits), rebuilt every call
     double* dc_part = nullptr;       // [DM_DC_BLOCKS] block sums of the k = 0 entry
+    float2* spec3 = nullptr;         // [n_k] forward spectrum recomputed for the PSF gradient (allocated on first use)
+    double* psfg_part = nullptr;     // [DM_PSFG_BLOCKS*6] block sums of the PSF gradient
+    float* psfg_out = nullptr;       // [6] device result of the PSF gradient
     int fwd_path = 0, bwd_path = 0;  // 0 = fast, 1 = robust
     float tau = 1e-2f, tau_b = 2e-4f;
     cufftHandle fft_xy = 0, fft_z = 0, fft_r2c = 0;
@@ -546,17 +549,33 @@ int dm_render_backward(dm_plan* p, const float* vertices_dev, const float* psf_c
                        float* dL_dvertices_dev, float* dL_dpsf_cov_host)
 {
     if (!p || !vertices_dev || !dL_dimage_dev || !dL_dvertices_dev) return DM_ERR_INVALID_ARG;
-    if (dL_dpsf_cov_host) return DM_ERR_UNSUPPORTED;
     if (p->ix_begin != 0 || p->ix_end != p->gd.nx) return DM_ERR_INVALID_ARG;
     DmPsfDev psf;
     int rc = make_psf(p, psf_cov_host, &psf);
     if (rc) return rc;
     if ((rc = ensure_fft(p))) return rc;
+    if (dL_dpsf_cov_host) {
+        const size_t nk = n_k_of(p);
+        if (!p->spec3 && cudaMalloc(&p->spec3, nk * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
+        if (!p->psfg_part && cudaMalloc(&p->psfg_part, DM_PSFG_BLOCKS * 6 * sizeof(double)) != cudaSuccess) return DM_ERR_ALLOC;
+        if (!p->psfg_out && cudaMalloc(&p->psfg_out, 6 * sizeof(float)) != cudaSuccess) return DM_ERR_ALLOC;
+    }
     stage_reset(p);
-    rc = run_image_to_cotangent(p, dL_dimage_dev, psf, (float*)p->spec2);
+    rc = run_image_to_cotangent(p, dL_dimage_dev, psf, (float*)p->spec2);   // leaves R = rfft3(dL/dimage) in p->spec
     if (rc) return rc;
     stage_begin(p, 0);
-    return run_backward(p, vertices_dev, (const float*)p->spec2, dL_dvertices_dev);
+    rc = run_backward(p, vertices_dev, (const float*)p->spec2, dL_dvertices_dev);
+    if (rc || !dL_dpsf_cov_host) return rc;
+    // PSF-parameter gradient: needs the forward spectrum F of these vertices (recomputed: one forward mesh FT)
+    if ((rc = run_forward(p, vertices_dev, (float*)p->spec3))) return rc;
+    dm_k_psf_grad_partial<<<DM_PSFG_BLOCKS, 256, 0, p->stream>>>(p->spec, p->spec3, p->gd, psf, p->psfg_part);
+    if ((rc = check_launch(p))) return rc;
+    dm_k_psf_grad_final<<<1, DM_PSFG_BLOCKS, 0, p->stream>>>(p->psfg_part, p->psfg_out);
+    if ((rc = check_launch(p))) return rc;
+    if (cudaMemcpyAsync(dL_dpsf_cov_host, p->psfg_out, 6 * sizeof(float), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+        cudaStreamSynchronize(p->stream) != cudaSuccess)
+        return DM_ERR_CUDA;
+    return DM_OK;
 }
 
 int dm_plan_stage_ms(dm_plan* p, float ms[4])
@@ -600,6 +619,9 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->fwd_part);
     cudaFree(p->hmax2);
     cudaFree(p->dc_part);
+    cudaFree(p->spec3);
+    cudaFree(p->psfg_part);
+    cudaFree(p->psfg_out);
     if (p->ev_ok)
         for (int i = 0; i < 8; ++i) cudaEventDestroy(p->ev[i]);
     delete p;

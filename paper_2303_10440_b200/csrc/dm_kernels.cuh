@@ -369,3 +369,58 @@ __global__ void dm_k_drop_selfconj_imag(float2* __restrict__ S, DmGridDev grid)
     S[(size_t)l * grid.nzh].y = 0.f;
     S[(size_t)l * grid.nzh + grid.nz / 2].y = 0.f;
 }
+
+// ---- PSF-parameter gradient (eq. 4 with reading R5) -----------------------------------------
+// dL/dSigma_m = sum_k q_m(k) w Re( conj(R) F c ),  q = (-kx^2/2, -ky^2/2, -kz^2/2, -kx ky, -kx kz, -ky kz),
+// R = rfft3(dL/dimage) (unnormalised; the 1/(N_tot h_x h_y h_z) rides on c), w as in dm_k_psf_adjoint.
+// Two stages with fixed-order fp64 tree reductions (deterministic): DM_PSFG_BLOCKS block sums of 6 numbers, then one block.
+#define DM_PSFG_BLOCKS 256
+__global__ void __launch_bounds__(256)
+dm_k_psf_grad_partial(const float2* __restrict__ R, const float2* __restrict__ F, DmGridDev grid, DmPsfDev psf,
+                      double* __restrict__ partial)
+{
+    __shared__ double sh[6][256];
+    const long long n = (long long)grid.nx * grid.ny * grid.nzh;
+    double acc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    for (long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (long long)gridDim.x * blockDim.x) {
+        const int iz = (int)(l % grid.nzh), iy = (int)((l / grid.nzh) % grid.ny), ix = (int)(l / ((long long)grid.nzh * grid.ny));
+        const cf c = dm_psf_coeff(grid, psf, ix, iy, iz);
+        const float2 f = F[l], r = R[l];
+        const float sre = f.x * c.re - f.y * c.im, sim = f.x * c.im + f.y * c.re;    // S = F c
+        const float w = (iz == 0 || iz == grid.nz / 2) ? 1.0f : 2.0f;
+        const double t = (double)(w * (r.x * sre + r.y * sim));                      // w Re(conj(R) S)
+        const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
+        const double kx = (double)(grid.kstep[0] * nx), ky = (double)(grid.kstep[1] * ny), kz = (double)(grid.kstep[2] * iz);
+        acc[0] -= 0.5 * kx * kx * t;
+        acc[1] -= 0.5 * ky * ky * t;
+        acc[2] -= 0.5 * kz * kz * t;
+        acc[3] -= kx * ky * t;
+        acc[4] -= kx * kz * t;
+        acc[5] -= ky * kz * t;
+    }
+#pragma unroll
+    for (int m = 0; m < 6; ++m) sh[m][threadIdx.x] = acc[m];
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (threadIdx.x < s)
+#pragma unroll
+            for (int m = 0; m < 6; ++m) sh[m][threadIdx.x] += sh[m][threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x < 6) partial[6 * blockIdx.x + threadIdx.x] = sh[threadIdx.x][0];
+}
+__global__ void __launch_bounds__(DM_PSFG_BLOCKS)
+dm_k_psf_grad_final(const double* __restrict__ partial, float* __restrict__ out6)
+{
+    __shared__ double sh[6][DM_PSFG_BLOCKS];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) sh[m][threadIdx.x] = partial[6 * threadIdx.x + m];
+    __syncthreads();
+    for (int s = DM_PSFG_BLOCKS / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s)
+#pragma unroll
+            for (int m = 0; m < 6; ++m) sh[m][threadIdx.x] += sh[m][threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x < 6) out6[threadIdx.x] = (float)sh[threadIdx.x][0];
+}

@@ -212,3 +212,28 @@ def test_error_codes(dm):
     plan = dm.Plan((8, 8, 8), (1 / 8,) * 3, (0, 0, 0), 0, torch.as_tensor(f, device="cuda"), v.shape[0])
     with pytest.raises(dm.DeltamicError):
         plan.set_slab(4, 4)
+
+
+def test_psf_gradient_cfg1_and_full_covariance(dm):
+    """NEXT 2: dL/dSigma from dm_render_backward against the oracle (relative error <= 1e-3 of the largest entry), with
+    config 1's diagonal PSF and with a full covariance on an anisotropic grid; the vertex gradient of the same call
+    must equal the one of a call without the PSF gradient, bit for bit."""
+    import torch
+    w = build_workload(1)
+    cases = [(w.n, w.spacing, w.origin, w.psf_cov.astype(np.float64)),
+             ((24, 32, 16), (1 / 24, 1 / 32, 1 / 8), (-0.5 + 1 / 48, -0.5 + 1 / 64, -1.0 + 1 / 16),
+              np.array([0.0020, 0.0016, 0.0300, 0.0004, -0.0015, 0.0011]))]
+    for n, spacing, origin, cov in cases:
+        for mode in (0, 1):
+            plan = dm.Plan(n, spacing, origin, mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+            vd = torch.as_tensor(w.vertices, device="cuda")
+            y = np.random.default_rng(3).standard_normal(n).astype(np.float32)
+            yd = torch.as_tensor(y, device="cuda")
+            dv0 = plan.render_backward(vd, cov, yd).clone()
+            dv, dcov = plan.render_backward(vd, cov, yd, with_psf_grad=True)
+            assert torch.equal(dv, dv0)
+            ref = oracle.render_backward_psf(w.vertices, w.faces, n, spacing, origin, cov, mode, y.astype(np.float64))
+            err = np.abs(np.array(dcov) - ref).max() / np.abs(ref).max()
+            print(f"psf gradient n={n} mode={mode}: max err / max|dL/dSigma| = {err:.2e}")
+            assert err <= 1e-3, (dcov, ref)
+            plan.close()
