@@ -76,6 +76,14 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
  * DESIGN.md section 9).  Default: the whole grid.  dm_render* require the whole grid. */
 int dm_plan_set_slab(dm_plan* plan, int32_t ix_begin, int32_t ix_end);
 
+/* Narrow band ("evaluate the FT only where the PSF spectrum is above 1 % of its maximum").
+ * With psf_cov_host = 6 floats on the HOST (covariance B of a Gaussian PSF, order xx, yy, zz, xy, xz, yz) and
+ * 0 < cutoff < 1, the mesh-FT calls of this plan evaluate only the stored frequencies with
+ * exp(-1/2 k^T B k) > cutoff: dm_mesh_ft_forward writes 0 everywhere else, dm_mesh_ft_backward ignores dL/dF there
+ * (the gradient of the banded forward).  dm_render* use the band too; B is normally the PSF they are called with.
+ * psf_cov_host = NULL switches the band off (the default).  k = 0 is always inside the band. */
+int dm_plan_set_narrow_band(dm_plan* plan, const float* psf_cov_host, float cutoff);
+
 /* Tuning / debugging knobs.  Defaults are the product path; the "robust" paths evaluate EVERY pair through the
  * series / far-pair branches (slow, used by the tests to cross-check the fast kernels at full size). */
 typedef enum dm_option {

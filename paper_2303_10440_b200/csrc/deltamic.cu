@@ -48,6 +48,8 @@ struct dm_plan {
     float2* fwd_part = nullptr;      // [st_n_chunks * n_k] per-chunk partial spectra
     unsigned int* hmax2 = nullptr;   // longest squared edge (float bits), rebuilt every call
     double* dc_part = nullptr;       // [DM_DC_BLOCKS] block sums of the k = 0 entry
+    int2* band_z = nullptr;          // [nx*ny] in-band z interval of every row (narrow band), valid while band_on
+    bool band_on = false;
     float2* spec3 = nullptr;         // [n_k] forward spectrum recomputed for the PSF gradient (allocated on first use)
     double* psfg_part = nullptr;     // [DM_PSFG_BLOCKS*6] block sums of the PSF gradient
     float* psfg_out = nullptr;       // [6] device result of the PSF gradient
@@ -100,6 +102,7 @@ int backward_splits(const dm_plan* p, int* rows_per_split)
     const int n_rows = (p->ix_end - p->ix_begin) * p->gd.ny;
     const int tri_blocks = (p->n_faces + 127) / 128;
     int want = (p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
+    if (p->band_on) want = p->n_split_max;   // rows differ in cost under the narrow band: many small CTAs balance the load
     if (want < 1) want = 1;
     if (want > n_rows) want = n_rows;
     if (want > p->n_split_max) want = p->n_split_max;
@@ -244,7 +247,7 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
             return DM_ERR_CUDA;                                                                                          \
         dm_k_backward_fast<MODE, SEG><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(                                     \
             p->btrec, p->bvrec, pt, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, p->tau_b, (const float2*)G_dev,      \
-            p->part);                                                                                                    \
+            p->band_on ? p->band_z : nullptr, p->part);                                                                                                    \
     } while (0)
         if (p->mode == DM_SURFACE) {
             if (seg == 8) DM_LAUNCH_BF(1, 8); else if (seg == 16) DM_LAUNCH_BF(1, 16); else DM_LAUNCH_BF(1, 32);
@@ -347,6 +350,8 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
         p->gd.kstep[d] = (float)(2.0 * M_PI / L);
         p->gd.inv_len[d] = 1.0 / L;
     }
+    for (int i = 0; i < 6; ++i) p->gd.band_cov[i] = 0.f;
+    p->gd.band_lim = INFINITY;
     p->ix_begin = 0;
     p->ix_end = p->gd.nx;
     // gap-product threshold of the fast path: one excluded-or-not pair may cost ~1e-6 (sum|d|)/tau of ONE triangle's
@@ -462,6 +467,26 @@ int dm_plan_set_slab(dm_plan* p, int32_t ix_begin, int32_t ix_end)
     p->ix_begin = ix_begin;
     p->ix_end = ix_end;
     return DM_OK;
+}
+
+int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
+{
+    if (!p) return DM_ERR_INVALID_ARG;
+    if (!psf_cov_host) {
+        p->band_on = false;
+        p->gd.band_lim = INFINITY;
+        return DM_OK;
+    }
+    if (!(cutoff > 0.f) || !(cutoff < 1.f)) return DM_ERR_INVALID_ARG;
+    for (int i = 0; i < 6; ++i)
+        if (!std::isfinite(psf_cov_host[i])) return DM_ERR_INVALID_ARG;
+    if (!p->band_z && cudaMalloc(&p->band_z, (size_t)p->gd.nx * p->gd.ny * sizeof(int2)) != cudaSuccess) return DM_ERR_ALLOC;
+    for (int i = 0; i < 6; ++i) p->gd.band_cov[i] = psf_cov_host[i];
+    p->gd.band_lim = std::log(1.0f / cutoff);
+    p->band_on = true;
+    const int n_rows = p->gd.nx * p->gd.ny;
+    dm_k_band_rows<<<(n_rows + 127) / 128, 128, 0, p->stream>>>(p->gd, p->band_z);
+    return check_launch(p);
 }
 
 int dm_plan_set_option(dm_plan* p, int option, double value)
@@ -619,6 +644,7 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->fwd_part);
     cudaFree(p->hmax2);
     cudaFree(p->dc_part);
+    cudaFree(p->band_z);
     cudaFree(p->spec3);
     cudaFree(p->psfg_part);
     cudaFree(p->psfg_out);

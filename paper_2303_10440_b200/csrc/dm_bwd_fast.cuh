@@ -191,7 +191,7 @@ template <int MODE, int SEG>
 __global__ void __launch_bounds__(DM_BF_THREADS, DM_BF_MINCTA)
 dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__ vrec_g, DmPatchDev pt, int n_faces,
                    DmGridDev grid, int ix_begin, int ix_end, int rows_per_split, float tau_b,
-                   const float2* __restrict__ G, float* __restrict__ part)
+                   const float2* __restrict__ G, const int2* __restrict__ band_z, float* __restrict__ part)
 {
     static_assert(SEG == 8 || SEG == 16 || SEG == 32, "SEG divides the 32-bit flag word");
     static_assert(DM_BF_UNR % DM_BF_STAGE == 0 && SEG % DM_BF_UNR == 0, "stages tile the unrolled body, bodies tile a segment");
@@ -248,7 +248,8 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         const float2* Grow = G + ((size_t)ix * grid.ny + iy) * nzh;
         for (int iz = tid; iz < nzh; iz += DM_BF_THREADS) {
             const float kz = grid.kstep[2] * iz;
-            const float2 Gk = Grow[iz];
+            float2 Gk = Grow[iz];
+            if (!dm_in_band(grid, nx, ny, iz)) Gk = make_float2(0.f, 0.f);  // narrow band: the cotangent outside is ignored
             float4 o;
             if (MODE == 1) {
                 o = make_float4(Gk.x, -Gk.y, kz, 0.f);                       // conj(G)
@@ -322,8 +323,15 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         const cf Xa = dm_expmi_turns((uint32_t)nx * uax + (uint32_t)ny * uay);
         DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
-        for (int zc = 0; zc < nzh; zc += DM_BF_CHUNK) {
-            const int clen = min(DM_BF_CHUNK, nzh - zc);
+        // narrow band: only the in-band interval of the row, started at a seed position
+        int z_lo = 0, z_hi = nzh;
+        if (band_z != nullptr) {
+            const int2 bz = band_z[ix * grid.ny + iy];
+            z_lo = bz.x & ~(SEG - 1);
+            z_hi = bz.y;
+        }
+        for (int zc = z_lo; zc < z_hi; zc += DM_BF_CHUNK) {
+            const int clen = min(DM_BF_CHUNK, z_hi - zc);
             uint32_t fl[DM_BF_CHUNK / 32];
             // ---- fast pass over the chunk: bodies of DM_BF_UNR frequencies, exact seeds every SEG ---------------------
             cf Ea = Xa;

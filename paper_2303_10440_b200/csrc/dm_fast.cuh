@@ -148,11 +148,12 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
 #pragma unroll
     for (int j = 0; j < DM_K; ++j) {
         kyj[j] = __fmul_rn(grid.kstep[1], (float)(nys0 + j));
-        const bool low = dm_k_is_low(grid, nx, nys0 + j, nz, hmax2);
+        const bool low = dm_k_is_low(grid, nx, nys0 + j, nz, hmax2) || !dm_in_band(grid, nx, nys0 + j, nz);
         tauj[j] = low ? -1.0f : tau;
         live |= !low;
     }
     live &= in_range;
+    if (!__syncthreads_or(live ? 1 : 0)) return;   // nothing to do for this block of frequencies (narrow band)
 
     float Fre[DM_K], Fim[DM_K];     // running sums (tile sums of the fast path + slow-path pairs)
     float C0[DM_K], C1[DM_K], dp[DM_K];
@@ -291,7 +292,7 @@ dm_k_forward_lowk(const float4* __restrict__ rec, const int32_t* __restrict__ ch
     if (nz > grid.nz / 2 || nys < -(grid.ny / 2) || nys > (grid.ny - 1) / 2 || nx < -(grid.nx / 2) || nx > (grid.nx - 1) / 2) return;
     const int ix = nx < 0 ? nx + grid.nx : nx, iy = nys < 0 ? nys + grid.ny : nys;
     if (ix < ix_begin || ix >= ix_end) return;
-    if (!dm_k_is_low(grid, nx, nys, nz, __uint_as_float(*hmax2_bits))) return;
+    if (!dm_k_is_low(grid, nx, nys, nz, __uint_as_float(*hmax2_bits)) || !dm_in_band(grid, nx, nys, nz)) return;
     const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * nys, kz = grid.kstep[2] * nz;
     float are = 0.f, aim = 0.f;
     for (int c = 0; c < n_chunks; ++c) {
@@ -340,8 +341,12 @@ __global__ void dm_k_forward_finish(const float2* __restrict__ part, size_t part
     const int iz = (int)(l % grid.nzh), iy = (int)((l / grid.nzh) % grid.ny);
     const int ix = ix_begin + (int)(l / ((long long)grid.nzh * grid.ny));
     const int nx = dm_signed_freq(ix, grid.nx), nys = dm_signed_freq(iy, grid.ny);
-    if (dm_k_is_low(grid, nx, nys, iz, __uint_as_float(*hmax2_bits))) return;
     const size_t o = ((size_t)ix * grid.ny + iy) * grid.nzh + iz;
+    if (!dm_in_band(grid, nx, nys, iz)) {   // narrow band: skipped entries are zero
+        F[o] = make_float2(0.f, 0.f);
+        return;
+    }
+    if (dm_k_is_low(grid, nx, nys, iz, __uint_as_float(*hmax2_bits))) return;
     float re = 0.f, im = 0.f;
     for (int c = 0; c < n_chunks; ++c) {
         const float2 v = part[(size_t)c * part_stride + o];

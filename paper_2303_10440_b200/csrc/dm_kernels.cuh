@@ -15,7 +15,19 @@ struct DmGridDev {
     int nx, ny, nz, nzh;      // voxels and nz/2+1
     float kstep[3];           // 2 pi / L_a
     double inv_len[3];        // 1 / L_a
+    // narrow band: only frequencies with 1/2 k^T B k < band_lim are evaluated (h_hat(k) > cutoff for
+    // the Gaussian PSF of covariance B, band_lim = ln(1/cutoff)); band_lim = +inf switches the band off
+    float band_cov[6];        // xx yy zz xy xz yz
+    float band_lim;
 };
+
+__device__ __forceinline__ bool dm_in_band(const DmGridDev& grid, int nx, int ny, int nz)
+{
+    const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny, kz = grid.kstep[2] * nz;
+    const float quad = grid.band_cov[0] * kx * kx + grid.band_cov[1] * ky * ky + grid.band_cov[2] * kz * kz +
+                       2.0f * (grid.band_cov[3] * kx * ky + grid.band_cov[4] * kx * kz + grid.band_cov[5] * ky * kz);
+    return 0.5f * quad < grid.band_lim;
+}
 
 __device__ __forceinline__ int dm_signed_freq(int i, int n) { return (i < (n + 1) / 2) ? i : i - n; }
 
@@ -142,7 +154,8 @@ dm_k_forward_robust(const float4* __restrict__ rec, int n_faces, DmGridDev grid,
     }
     if (live) {
         const size_t o = ((size_t)ix * grid.ny + iy) * grid.nzh + iz;
-        // volume mode carries the factor i of (i/|k|^2)
+        // volume mode carries the factor i of (i/|k|^2); entries outside the narrow band are zero
+        if (!dm_in_band(grid, nx, ny, nz)) acc_re = acc_im = 0.f;
         F[o] = (mode == 1) ? make_float2(acc_re, acc_im) : make_float2(-acc_im, acc_re);
     }
 }
@@ -183,7 +196,8 @@ dm_k_backward_robust(const float4* __restrict__ rec, int n_faces, DmGridDev grid
         for (int s = 0; s < DM_BWD_NSUM; ++s) racc[s] = 0.f;
         for (int iz = 0; iz < grid.nzh; ++iz) {
             const float kz = grid.kstep[2] * iz;
-            const float2 Gk = Grow[iz];
+            float2 Gk = Grow[iz];
+            if (!dm_in_band(grid, nx, ny, iz)) Gk = make_float2(0.f, 0.f);   // narrow band
             const float k2 = kx * kx + ky * ky + kz * kz;
             cf kappa;
             float omega;
@@ -423,4 +437,22 @@ dm_k_psf_grad_final(const double* __restrict__ partial, float* __restrict__ out6
         __syncthreads();
     }
     if (threadIdx.x < 6) out6[threadIdx.x] = (float)sh[threadIdx.x][0];
+}
+
+// ---- narrow band: the in-band interval [z_lo, z_hi) of every (i_x, i_y) row ----------------------
+// (the band is convex, so the in-band frequencies of a row are contiguous; an empty row gets z_lo = z_hi = 0)
+__global__ void dm_k_band_rows(DmGridDev grid, int2* __restrict__ band_z)
+{
+    const int row = blockIdx.x * blockDim.x + threadIdx.x;
+    if (row >= grid.nx * grid.ny) return;
+    const int nx = dm_signed_freq(row / grid.ny, grid.nx), ny = dm_signed_freq(row % grid.ny, grid.ny);
+    int lo = 0, hi = 0;
+    bool any = false;
+    for (int iz = 0; iz < grid.nzh; ++iz)
+        if (dm_in_band(grid, nx, ny, iz)) {
+            if (!any) lo = iz;
+            any = true;
+            hi = iz + 1;
+        }
+    band_z[row] = make_int2(lo, hi);
 }

@@ -237,3 +237,52 @@ def test_psf_gradient_cfg1_and_full_covariance(dm):
             print(f"psf gradient n={n} mode={mode}: max err / max|dL/dSigma| = {err:.2e}")
             assert err <= 1e-3, (dcov, ref)
             plan.close()
+
+
+def _band_mask(w, cov, cutoff):
+    """In-band mask of the stored grid in fp64 and the mask of frequencies too close to the boundary to call."""
+    k = oracle.frequency_grid(w.n, w.spacing)
+    S = np.array([[cov[0], cov[3], cov[4]], [cov[3], cov[1], cov[5]], [cov[4], cov[5], cov[2]]], dtype=np.float64)
+    quad = 0.5 * np.einsum("...i,ij,...j->...", k, S, k)
+    lim = np.log(1.0 / cutoff)
+    return quad < lim, np.abs(quad - lim) < 1e-4 * lim
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_narrow_band_forward_and_backward(dm, mode):
+    """NEXT 1: with the band set, the forward equals the oracle inside the band and is exactly zero
+    outside; the backward equals the oracle's gradient summed over the in-band frequencies only.  Anisotropic grid and
+    a full covariance, so the band is a tilted ellipsoid cut by the grid."""
+    import torch
+    w = build_workload(2, subdiv_override=2, grid_override=(24, 32, 40))
+    cov = np.array([1.2e-3, 0.7e-3, 4.5e-3, 2.0e-4, -0.8e-3, 3.0e-4])
+    cutoff = 0.02
+    inb, edge = _band_mask(w, cov, cutoff)
+    assert 0.03 < inb.mean() < 0.7 and inb[0, 0, 0]
+    plan, vd = _plan(dm, w, mode), _dev(w.vertices)
+    plan.set_narrow_band(cov, cutoff)
+    F = plan.mesh_ft_forward(vd).cpu().numpy()
+    ref = oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, mode)
+    f0 = abs(ref[0, 0, 0])
+    sure_in, sure_out = inb & ~edge, ~inb & ~edge
+    assert np.abs(F - ref)[sure_in].max() <= FWD_TOL * f0
+    assert (F[sure_out] == 0).all()
+    G = spectrum_cotangent(w)
+    G[edge] = 0
+    dv = plan.mesh_ft_backward(vd, _dev(G)).cpu().numpy()
+    idx = np.nonzero(sure_in.reshape(-1))[0]
+    dref = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, mode, G.reshape(-1)[idx].astype(np.complex128),
+                                        flat_indices=idx)
+    assert _rel_l2(dv, dref) <= GRAD_TOL
+    # the robust kernels honour the band too
+    plan.set_option(dm.DM_OPT_FORWARD_PATH, 1)
+    plan.set_option(dm.DM_OPT_BACKWARD_PATH, 1)
+    Fr = plan.mesh_ft_forward(vd).cpu().numpy()
+    assert np.abs(Fr - ref)[sure_in].max() <= FWD_TOL * f0 and (Fr[sure_out] == 0).all()
+    assert _rel_l2(plan.mesh_ft_backward(vd, _dev(G)).cpu().numpy(), dref) <= GRAD_TOL
+    # switching the band off restores the whole grid
+    plan.set_option(dm.DM_OPT_FORWARD_PATH, 0)
+    plan.set_narrow_band(None)
+    F2 = plan.mesh_ft_forward(vd).cpu().numpy()
+    assert np.abs(F2 - ref).max() <= FWD_TOL * f0
+    plan.close()
