@@ -180,7 +180,7 @@ int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
     int rc = check_launch(p);
     if (rc) return rc;
     const int n_yruns = (p->gd.ny + DM_K - 1) / DM_K;
-    const long long n_thr = (long long)(p->ix_end - p->ix_begin) * n_yruns * p->gd.nzh;
+    const long long n_thr = (long long)(p->ix_end - p->ix_begin) * n_yruns * p->gd.nzb;
     dim3 grid((unsigned)((n_thr + DM_FAST_THREADS - 1) / DM_FAST_THREADS), (unsigned)p->st_n_chunks);
     const size_t stride = n_k_of(p);
     if (p->mode == DM_SURFACE)
@@ -352,6 +352,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
     }
     for (int i = 0; i < 6; ++i) p->gd.band_cov[i] = 0.f;
     p->gd.band_lim = INFINITY;
+    p->gd.nzb = p->gd.nzh;
     p->ix_begin = 0;
     p->ix_end = p->gd.nx;
     // gap-product threshold of the fast path: one excluded-or-not pair may cost ~1e-6 (sum|d|)/tau of ONE triangle's
@@ -475,6 +476,7 @@ int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
     if (!psf_cov_host) {
         p->band_on = false;
         p->gd.band_lim = INFINITY;
+        p->gd.nzb = p->gd.nzh;
         return DM_OK;
     }
     if (!(cutoff > 0.f) || !(cutoff < 1.f)) return DM_ERR_INVALID_ARG;
@@ -484,6 +486,20 @@ int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
     for (int i = 0; i < 6; ++i) p->gd.band_cov[i] = psf_cov_host[i];
     p->gd.band_lim = std::log(1.0f / cutoff);
     p->band_on = true;
+    // extent of the band ellipsoid along z: k_z^2 <= 2 L (B^-1)_zz; two frequencies of margin, the whole axis when B is
+    // not positive definite
+    {
+        const double xx = psf_cov_host[0], yy = psf_cov_host[1], zz = psf_cov_host[2], xy = psf_cov_host[3],
+                     xz = psf_cov_host[4], yz = psf_cov_host[5];
+        const double det = xx * (yy * zz - yz * yz) - xy * (xy * zz - yz * xz) + xz * (xy * yz - yy * xz);
+        const double cof = xx * yy - xy * xy;
+        p->gd.nzb = p->gd.nzh;
+        if (det > 0.0 && cof > 0.0 && xx > 0.0) {
+            const double kz_max = std::sqrt(2.0 * (double)p->gd.band_lim * cof / det);
+            const double nz_max = kz_max / (double)p->gd.kstep[2];
+            if (nz_max + 3.0 < (double)p->gd.nzh) p->gd.nzb = (int)nz_max + 3;
+        }
+    }
     const int n_rows = p->gd.nx * p->gd.ny;
     dm_k_band_rows<<<(n_rows + 127) / 128, 128, 0, p->stream>>>(p->gd, p->band_z);
     return check_launch(p);

@@ -19,6 +19,7 @@ struct DmGridDev {
     // the Gaussian PSF of covariance B, band_lim = ln(1/cutoff)); band_lim = +inf switches the band off
     float band_cov[6];        // xx yy zz xy xz yz
     float band_lim;
+    int nzb;                  // stored z-frequencies 0..nzb-1 can be inside the band (nzb = nzh when the band is off)
 };
 
 __device__ __forceinline__ bool dm_in_band(const DmGridDev& grid, int nx, int ny, int nz)
@@ -26,7 +27,7 @@ __device__ __forceinline__ bool dm_in_band(const DmGridDev& grid, int nx, int ny
     const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny, kz = grid.kstep[2] * nz;
     const float quad = grid.band_cov[0] * kx * kx + grid.band_cov[1] * ky * ky + grid.band_cov[2] * kz * kz +
                        2.0f * (grid.band_cov[3] * kx * ky + grid.band_cov[4] * kx * kz + grid.band_cov[5] * ky * kz);
-    return 0.5f * quad < grid.band_lim;
+    return nz < grid.nzb && 0.5f * quad < grid.band_lim;
 }
 
 __device__ __forceinline__ int dm_signed_freq(int i, int n) { return (i < (n + 1) / 2) ? i : i - n; }
