@@ -18,6 +18,9 @@ from .mesh_ft import (  # noqa: F401
     mesh_ft_forward_grid,
     mesh_ft_backward,
     mesh_ft_backward_grid,
+    mesh_ft_backward_normalised,
+    mesh_ft_forward_normalised,
+    surface_area_and_gradient,
     num_threads,
 )
 from .render import (psf_shift_spectrum, render, render_backward, render_backward_psf, spectrum_to_image,  # noqa: F401

@@ -130,3 +130,41 @@ def mesh_ft_backward_grid(vertices, faces, n, spacing, mode: int, G, flat_indice
     if flat_indices is not None:
         return mesh_ft_backward(vertices, faces, kg[np.asarray(flat_indices)], mode, G)
     return mesh_ft_backward(vertices, faces, kg, mode, np.asarray(G).reshape(-1))
+
+
+# ---- area-normalised membrane density (eq. 12-13; NEXT 3) ------------------------------------------------
+def surface_area_and_gradient(vertices, faces):
+    """|Lambda| = sum_T A_T and d|Lambda|/dv [n_V,3] = sum over the vertex star of dA_T/dv_p = -w_p/2, w_p = e_p x N_T,
+    e_p = v_{p-} - v_{p+}.  Degenerate triangles contribute 0 (reading R19)."""
+    v, f = _prep(vertices, faces)
+    area, grad = 0.0, np.zeros_like(v)
+    for tri in f:
+        p = v[tri]
+        m = np.cross(p[1] - p[0], p[2] - p[0])
+        mn = float(np.linalg.norm(m))
+        area += 0.5 * mn
+        if mn < 1e-30:
+            continue
+        N = m / mn
+        for c in range(3):
+            e = p[(c + 2) % 3] - p[(c + 1) % 3]
+            grad[tri[c]] += -0.5 * np.cross(e, N)
+    return area, grad
+
+
+def mesh_ft_forward_normalised(vertices, faces, kvec) -> np.ndarray:
+    """eq. 12: u_Lambda(k) = (1/|Lambda|) sum_T 2 A_T f_T(k) -- the surface-mode FT divided by the total area."""
+    area, _ = surface_area_and_gradient(vertices, faces)
+    return mesh_ft_forward(vertices, faces, kvec, 1) / area
+
+
+def mesh_ft_backward_normalised(vertices, faces, kvec, G) -> np.ndarray:
+    """eq. 13: the gradient of eq. 12 by the quotient rule,
+        dL/dv = (1/|Lambda|) sum_k Re(conj(G) dF/dv) - ( sum_k Re(conj(G) u_Lambda(k)) / |Lambda| ) d|Lambda|/dv ,
+    F the un-normalised surface-mode FT."""
+    area, darea = surface_area_and_gradient(vertices, faces)
+    Gc = np.asarray(G, dtype=np.complex128).reshape(-1)
+    bare = mesh_ft_backward(vertices, faces, kvec, 1, Gc)
+    u = mesh_ft_forward(vertices, faces, kvec, 1) / area
+    s = float((np.conj(Gc) * u).real.sum())
+    return bare / area - (s / area) * darea

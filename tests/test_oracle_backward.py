@@ -111,3 +111,33 @@ def test_degenerate_triangle_contributes_zero_in_surface_mode():
     g1 = oracle.mesh_ft_backward(v, f, k, SURF, G)
     g2 = oracle.mesh_ft_backward(v2, f2, k, SURF, G)
     assert np.abs(g2[:8] - g1).max() < 1e-15 and np.all(g2[8] == 0)
+
+
+def test_area_normalised_density_eq12_eq13():
+    """NEXT 3: the area gradient -w_p/2 against central differences of the area, and
+    the gradient of the normalised FT (eq. 13) against central differences of eq. 12; u_Lambda(0) = 1; scale invariance
+    u_{s Lambda}(k) = u_Lambda(s k)."""
+    from workloads import icosphere
+    rng = np.random.default_rng(21)
+    v, f = icosphere(1, 0.3, (0.03, -0.02, 0.01))
+    v = (v + 0.02 * rng.standard_normal(v.shape)).astype(np.float32).astype(np.float64)
+    k = rng.uniform(-25, 25, size=(40, 3))
+    k[0] = 0.0
+    G = rng.standard_normal(40) + 1j * rng.standard_normal(40)
+    area, darea = oracle.surface_area_and_gradient(v, f)
+    u = oracle.mesh_ft_forward_normalised(v, f, k)
+    assert abs(u[0] - 1.0) < 1e-14
+    assert np.abs(oracle.mesh_ft_forward_normalised(1.7 * v, f, k / 1.7) - u).max() < 1e-13
+    grad = oracle.mesh_ft_backward_normalised(v, f, k, G)
+    fd, fda = np.zeros_like(v), np.zeros_like(v)
+    h = 1e-6
+    for i in range(v.shape[0]):
+        for d in range(3):
+            vp, vm = v.copy(), v.copy()
+            vp[i, d] += h
+            vm[i, d] -= h
+            fd[i, d] = ((np.conj(G) * oracle.mesh_ft_forward_normalised(vp, f, k)).real.sum()
+                        - (np.conj(G) * oracle.mesh_ft_forward_normalised(vm, f, k)).real.sum()) / (2 * h)
+            fda[i, d] = (oracle.surface_area_and_gradient(vp, f)[0] - oracle.surface_area_and_gradient(vm, f)[0]) / (2 * h)
+    assert np.linalg.norm(darea - fda) <= 1e-8 * np.linalg.norm(fda)
+    assert np.linalg.norm(grad - fd) <= 1e-7 * np.linalg.norm(fd)
