@@ -6,6 +6,7 @@ streams.  There is no CPU fallback: importing the binding without the built libr
 device, raises.
 """
 from ._binding import (  # noqa: F401
+    DM_OPT_AREA_NORMALISED,
     DM_OPT_BACKWARD_PATH,
     DM_OPT_FORWARD_PATH,
     DM_OPT_TAU,

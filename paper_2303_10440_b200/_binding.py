@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(HERE, "libdeltamic.so")
 
 DM_VOLUME, DM_SURFACE = 0, 1
-DM_OPT_FORWARD_PATH, DM_OPT_BACKWARD_PATH, DM_OPT_TAU, DM_OPT_TAU_BWD = 0, 1, 2, 3
+DM_OPT_FORWARD_PATH, DM_OPT_BACKWARD_PATH, DM_OPT_TAU, DM_OPT_TAU_BWD, DM_OPT_AREA_NORMALISED = 0, 1, 2, 3, 4
 
 # every symbol include/deltamic.h declares
 _SYMBOLS = (

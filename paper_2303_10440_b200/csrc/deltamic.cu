@@ -48,6 +48,9 @@ struct dm_plan {
     float2* fwd_part = nullptr;      // [st_n_chunks * n_k] per-chunk partial spectra
     unsigned int* hmax2 = nullptr;   // longest squared edge (float bits), rebuilt every call
     double* dc_part = nullptr;       // [DM_DC_BLOCKS] block sums of the k = 0 entry
+    bool normalise = false;          // DM_OPT_AREA_NORMALISED (surface mode): u = F/|Lambda|, eq. 12-13
+    double* dc_total = nullptr;      // [1] fp64 volume / total area of the last forward (k = 0 kernels)
+    double* dot_part = nullptr;      // [DM_DOT_BLOCKS + 1] block sums and result of sum_k Re(conj(G) F)
     int2* band_z = nullptr;          // [nx*ny] in-band z interval of every row (narrow band), valid while band_on
     bool band_on = false;
     float2* spec3 = nullptr;         // [n_k] forward spectrum recomputed for the PSF gradient (allocated on first use)
@@ -205,17 +208,28 @@ int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
     return check_launch(p);
 }
 
-int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
+int run_forward_raw(dm_plan* p, const float* vertices_dev, float* F_dev)
 {
     int rc = p->fwd_path == 0 ? run_forward_fast(p, vertices_dev, F_dev) : run_forward_robust(p, vertices_dev, F_dev);
     if (rc) return rc;
     if (p->ix_begin == 0) {
         dm_k_dc_partial<<<DM_DC_BLOCKS, 256, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode, p->dc_part);
         if ((rc = check_launch(p))) return rc;
-        dm_k_dc_final<<<1, DM_DC_BLOCKS, 0, p->stream>>>(p->dc_part, F_dev);
+        dm_k_dc_final<<<1, DM_DC_BLOCKS, 0, p->stream>>>(p->dc_part, F_dev, p->dc_total);
         rc = check_launch(p);
     }
     return rc;
+}
+
+// forward as the caller sees it: the raw mesh FT, divided by the total area in the area-normalised mode (eq. 12)
+int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
+{
+    if (p->normalise && (p->ix_begin != 0 || p->ix_end != p->gd.nx)) return DM_ERR_UNSUPPORTED;
+    int rc = run_forward_raw(p, vertices_dev, F_dev);
+    if (rc || !p->normalise) return rc;
+    const long long nk = (long long)n_k_of(p);
+    dm_k_scale_spectrum<<<(unsigned)((nk + 255) / 256), 256, 0, p->stream>>>((float2*)F_dev, nk, p->dc_total);
+    return check_launch(p);
 }
 
 int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, float* dv_dev)
@@ -263,10 +277,25 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     rc = check_launch(p);
     if (rc) return rc;
     stage_end(p, 0);
+    const double *area_total = nullptr, *sdot = nullptr;
+    if (p->normalise) {
+        // eq. 13's second term needs |Lambda| and sum_k Re(conj(G) F): one raw forward of these vertices and a dot product
+        if (p->ix_begin != 0 || p->ix_end != p->gd.nx) return DM_ERR_UNSUPPORTED;
+        const long long nk = (long long)n_k_of(p);
+        if (!p->spec3 && cudaMalloc(&p->spec3, (size_t)nk * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
+        if (!p->dot_part && cudaMalloc(&p->dot_part, (DM_DOT_BLOCKS + 1) * sizeof(double)) != cudaSuccess) return DM_ERR_ALLOC;
+        if ((rc = run_forward_raw(p, vertices_dev, (float*)p->spec3))) return rc;
+        dm_k_dot_partial<<<DM_DOT_BLOCKS, 256, 0, p->stream>>>((const float2*)G_dev, p->spec3, nk, p->dot_part);
+        if ((rc = check_launch(p))) return rc;
+        dm_k_dot_final<<<1, DM_DOT_BLOCKS, 0, p->stream>>>(p->dot_part, p->dot_part + DM_DOT_BLOCKS);
+        if ((rc = check_launch(p))) return rc;
+        area_total = p->dc_total;
+        sdot = p->dot_part + DM_DOT_BLOCKS;
+    }
     stage_begin(p, 3);
     dm_k_corner_grads<<<(p->n_faces + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode,
                                                                        n_split, p->part, (const float2*)G_dev,
-                                                                       p->ix_begin == 0 ? 1 : 0, p->corner);
+                                                                       p->ix_begin == 0 ? 1 : 0, area_total, sdot, p->corner);
     rc = check_launch(p);
     if (rc) return rc;
     dm_k_vertex_gather<<<(p->n_vertices + 127) / 128, 128, 0, p->stream>>>(p->csr_off, p->csr_corner, p->n_vertices,
@@ -416,7 +445,8 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
                 cudaMalloc(&p->st_rec, (size_t)p->st_n_rec * 3 * sizeof(float4)) != cudaSuccess ||
                 cudaMalloc(&p->fwd_part, (size_t)p->st_n_chunks * nk * sizeof(float2)) != cudaSuccess ||
                 cudaMalloc(&p->hmax2, sizeof(unsigned int)) != cudaSuccess ||
-                cudaMalloc(&p->dc_part, DM_DC_BLOCKS * sizeof(double)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
+                cudaMalloc(&p->dc_part, DM_DC_BLOCKS * sizeof(double)) != cudaSuccess ||
+                cudaMalloc(&p->dc_total, sizeof(double)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
             if (cudaMemcpyAsync(p->st_new, sr.vid_new.data(), nb, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
                 cudaMemcpyAsync(p->st_prev, sr.vid_prev.data(), nb, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
                 cudaMemcpyAsync(p->st_ret, sr.vid_ret.data(), nb, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
@@ -520,6 +550,10 @@ int dm_plan_set_option(dm_plan* p, int option, double value)
         case DM_OPT_TAU:
             if (!(value >= 0.0) || !std::isfinite(value)) return DM_ERR_INVALID_ARG;
             p->tau = (float)value;
+            return DM_OK;
+        case DM_OPT_AREA_NORMALISED:
+            if ((value != 0.0 && value != 1.0) || (value == 1.0 && p->mode != DM_SURFACE)) return DM_ERR_INVALID_ARG;
+            p->normalise = value == 1.0;
             return DM_OK;
         case DM_OPT_TAU_BWD:
             if (!(value >= 0.0) || !std::isfinite(value)) return DM_ERR_INVALID_ARG;
@@ -660,6 +694,8 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->fwd_part);
     cudaFree(p->hmax2);
     cudaFree(p->dc_part);
+    cudaFree(p->dc_total);
+    cudaFree(p->dot_part);
     cudaFree(p->band_z);
     cudaFree(p->spec3);
     cudaFree(p->psfg_part);

@@ -91,7 +91,7 @@ dm_k_dc_partial(const float* __restrict__ vertices, const int32_t* __restrict__ 
     if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
 }
 __global__ void __launch_bounds__(DM_DC_BLOCKS)
-dm_k_dc_final(const double* __restrict__ partial, float* __restrict__ F0)
+dm_k_dc_final(const double* __restrict__ partial, float* __restrict__ F0, double* __restrict__ total)
 {
     __shared__ double sh[DM_DC_BLOCKS];
     sh[threadIdx.x] = partial[threadIdx.x];
@@ -103,6 +103,7 @@ dm_k_dc_final(const double* __restrict__ partial, float* __restrict__ F0)
     if (threadIdx.x == 0) {
         F0[0] = (float)sh[0];
         F0[1] = 0.f;
+        *total = sh[0];   // volume or total area |Lambda| in fp64, kept for the area-normalised density (eq. 12)
     }
 }
 
@@ -250,7 +251,8 @@ dm_k_backward_robust(const float4* __restrict__ rec, int n_faces, DmGridDev grid
 //   V_a = W - V_b - V_c.   Degenerate triangle in surface mode contributes 0 (reading R19).
 __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int32_t* __restrict__ faces, int n_faces,
                                   int mode, int n_split, const float* __restrict__ part,
-                                  const float2* __restrict__ G, int has_dc, float* __restrict__ corner)
+                                  const float2* __restrict__ G, int has_dc, const double* __restrict__ area_total,
+                                  const double* __restrict__ sdot, float* __restrict__ corner)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n_faces) return;
@@ -260,6 +262,15 @@ __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int3
     for (int sp = 0; sp < n_split; ++sp)
 #pragma unroll
         for (int j = 0; j < DM_BWD_NSUM; ++j) s[j] += part[((size_t)sp * DM_BWD_NSUM + j) * n_faces + t];
+    if (area_total != nullptr) {
+        // area-normalised density u = F/|Lambda| (eq. 12-13): the sums were taken with the cotangent G of
+        // u, so  dL/dv = (1/|Lambda|) bare - (S/|Lambda|) d|Lambda|/dv,  S = sum_k Re(conj(G) u) = sdot/|Lambda|, and
+        // d|Lambda|/dv_p = -w_p/2 folds into the coefficient of -w_p:  S0 -> S0/|Lambda| - S/(2|Lambda|)
+        const double inv = 1.0 / *area_total;
+#pragma unroll
+        for (int j = 0; j < DM_BWD_NSUM; ++j) s[j] = (float)((double)s[j] * inv);
+        s[0] = (float)((double)s[0] - 0.5 * (*sdot) * inv * inv);
+    }
     const int idx[3] = {faces[3 * t], faces[3 * t + 1], faces[3 * t + 2]};
     float v[3][3];
 #pragma unroll
@@ -456,4 +467,48 @@ __global__ void dm_k_band_rows(DmGridDev grid, int2* __restrict__ band_z)
             hi = iz + 1;
         }
     band_z[row] = make_int2(lo, hi);
+}
+
+// ---- area-normalised membrane density (eq. 12-13) -----------------------------------------------------
+// u = F / |Lambda|: scale the spectrum by the fp64 total area the k = 0 kernels left in *total
+__global__ void dm_k_scale_spectrum(float2* __restrict__ F, long long n, const double* __restrict__ total)
+{
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= n) return;
+    const float inv = (float)(1.0 / *total);
+    float2 f = F[l];
+    f.x *= inv;
+    f.y *= inv;
+    F[l] = f;
+}
+// sdot = sum_k Re(conj(G) F) over the stored entries, fp64, two fixed-order stages
+#define DM_DOT_BLOCKS 256
+__global__ void __launch_bounds__(256)
+dm_k_dot_partial(const float2* __restrict__ G, const float2* __restrict__ F, long long n, double* __restrict__ partial)
+{
+    __shared__ double sh[256];
+    double acc = 0.0;
+    for (long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (long long)gridDim.x * blockDim.x) {
+        const float2 g = G[l], f = F[l];
+        acc += (double)g.x * (double)f.x + (double)g.y * (double)f.y;
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+__global__ void __launch_bounds__(DM_DOT_BLOCKS)
+dm_k_dot_final(const double* __restrict__ partial, double* __restrict__ out)
+{
+    __shared__ double sh[DM_DOT_BLOCKS];
+    sh[threadIdx.x] = partial[threadIdx.x];
+    __syncthreads();
+    for (int s = DM_DOT_BLOCKS / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sh[0];
 }

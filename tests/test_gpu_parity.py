@@ -286,3 +286,22 @@ def test_narrow_band_forward_and_backward(dm, mode):
     F2 = plan.mesh_ft_forward(vd).cpu().numpy()
     assert np.abs(F2 - ref).max() <= FWD_TOL * f0
     plan.close()
+
+
+def test_area_normalised_density_eq12_eq13(dm):
+    """NEXT 3: u = F/|Lambda| and its gradient against the oracle on a full small grid."""
+    w = build_workload(2, subdiv_override=2, grid_override=(16, 16, 16))
+    plan, vd = _plan(dm, w, 1), _dev(w.vertices)
+    plan.set_option(dm.DM_OPT_AREA_NORMALISED, 1)
+    k = oracle.frequency_grid(w.n, w.spacing).reshape(-1, 3)
+    u = plan.mesh_ft_forward(vd).cpu().numpy()
+    uref = oracle.mesh_ft_forward_normalised(w.vertices, w.faces, k).reshape(u.shape)
+    assert abs(u[0, 0, 0] - 1.0) <= 1e-6
+    assert np.abs(u - uref).max() <= FWD_TOL          # |u(0)| = 1
+    G = spectrum_cotangent(w)
+    dv = plan.mesh_ft_backward(vd, _dev(G)).cpu().numpy()
+    dref = oracle.mesh_ft_backward_normalised(w.vertices, w.faces, k, G.reshape(-1).astype(np.complex128))
+    assert _rel_l2(dv, dref) <= GRAD_TOL
+    plan.close()
+    with pytest.raises(dm.DeltamicError):             # volume mode has no area normalisation
+        _plan(dm, w, 0).set_option(dm.DM_OPT_AREA_NORMALISED, 1)
