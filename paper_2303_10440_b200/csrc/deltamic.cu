@@ -252,7 +252,7 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     if (p->bwd_path == 0 && nzh <= 288) {
         const DmPatchDev pt = {p->pt_face, p->pt_vid, p->pt_loc, p->pt_lanes};
         grid.x = (unsigned)(p->pt_lanes / DM_BF_THREADS);
-        dm_k_bwd_geometry<<<p->pt_lanes / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, pt, p->gd, p->btrec, p->bvrec);
+        dm_k_bwd_geometry<<<(p->pt_lanes + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, pt, p->gd, p->btrec, p->bvrec);
         if ((rc = check_launch(p))) return rc;
 #define DM_LAUNCH_BF(MODE, SEG)                                                                                          \
     do {                                                                                                                 \

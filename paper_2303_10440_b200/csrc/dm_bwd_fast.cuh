@@ -40,7 +40,9 @@
 #include "dm_kernels.cuh"
 #include "dm_patches.h"
 
+#ifndef DM_BF_THREADS
 #define DM_BF_THREADS 128
+#endif
 #ifndef DM_BF_MINCTA
 #define DM_BF_MINCTA 5         // resident CTAs per SM the register allocation aims at (<= 102 registers)
 #endif
