@@ -27,7 +27,9 @@
 static_assert(DM_STRIP_UNROLL == 6, "the strip loop is unrolled by 6 (window period 3 x gap ping-pong 2)");
 #define DM_K 8                      // frequencies per thread (run along y)
 #define DM_FAST_THREADS 128
-#define DM_FAST_TILE 192            // strip records per shared-memory tile (multiple of DM_STRIP_UNROLL and of 32)
+#ifndef DM_FAST_TILE
+#define DM_FAST_TILE 384            // strip records per shared-memory tile (multiple of DM_STRIP_UNROLL and of 32)
+#endif
 #define DM_LOWK_RADIUS 0.5f         // |k| h_max below which a frequency is "low" (all gaps small for all triangles)
 #define DM_LOWK_BOX 24              // low-k kernel covers |n_a| <= DM_LOWK_BOX
 
