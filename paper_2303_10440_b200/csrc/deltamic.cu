@@ -254,20 +254,25 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
         grid.x = (unsigned)(p->pt_lanes / DM_BF_THREADS);
         dm_k_bwd_geometry<<<(p->pt_lanes + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, pt, p->gd, p->btrec, p->bvrec);
         if ((rc = check_launch(p))) return rc;
-#define DM_LAUNCH_BF(MODE, SEG)                                                                                          \
+#define DM_LAUNCH_BF2(MODE, SEG, BAND)                                                                                   \
     do {                                                                                                                 \
-        if (cudaFuncSetAttribute(dm_k_backward_fast<MODE, SEG>, cudaFuncAttributeMaxDynamicSharedMemorySize,             \
+        if (cudaFuncSetAttribute(dm_k_backward_fast<MODE, SEG, BAND>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
                                  (int)row_smem) != cudaSuccess)                                                          \
             return DM_ERR_CUDA;                                                                                          \
-        dm_k_backward_fast<MODE, SEG><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(                                     \
+        dm_k_backward_fast<MODE, SEG, BAND><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(                               \
             p->btrec, p->bvrec, pt, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, p->tau_b, (const float2*)G_dev,      \
-            p->band_on ? p->band_z : nullptr, p->part);                                                                                                    \
+            p->band_z, p->part);                                                                                         \
+    } while (0)
+#define DM_LAUNCH_BF(MODE, SEG)                                                                                          \
+    do {                                                                                                                 \
+        if (p->band_on) DM_LAUNCH_BF2(MODE, SEG, true); else DM_LAUNCH_BF2(MODE, SEG, false);                            \
     } while (0)
         if (p->mode == DM_SURFACE) {
             if (seg == 8) DM_LAUNCH_BF(1, 8); else if (seg == 16) DM_LAUNCH_BF(1, 16); else DM_LAUNCH_BF(1, 32);
         } else {
             if (seg == 8) DM_LAUNCH_BF(0, 8); else if (seg == 16) DM_LAUNCH_BF(0, 16); else DM_LAUNCH_BF(0, 32);
         }
+#undef DM_LAUNCH_BF2
 #undef DM_LAUNCH_BF
     } else {
         if ((rc = run_geometry(p, vertices_dev))) return rc;

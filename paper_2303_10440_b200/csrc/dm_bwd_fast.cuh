@@ -180,7 +180,8 @@ __device__ __forceinline__ bool dm_bf_pair(const float kz, const cf A0, const cf
 
 // ---- A6 backward, fast kernel -----------------------------------------------------------------------------------
 // grid = (n_lanes / DM_BF_THREADS, n_split): one warp per patch; part[(split*13 + s)*n_faces + face] as in
-// dm_k_backward_robust.  SEG = frequencies between exact phase seeds (8, 16 or 32; chosen by the host so that the seed
+// dm_k_backward_robust.  BAND = the narrow band is set (band_z holds the in-band z interval of every row).
+// SEG = frequencies between exact phase seeds (8, 16 or 32; chosen by the host so that the seed
 // table fits).  Dynamic shared memory:
 //   2 * nzh float4                      double-buffered rows (kappa.re, kappa.im, k_z, -)
 //   (nseg-1) * 128 float2               seed table ztab[a-1][tid] = e^{-2 pi i (a SEG) u_z} of the thread's vertex
@@ -189,7 +190,7 @@ __device__ __forceinline__ bool dm_bf_pair(const float kz, const cf A0, const cf
 //                                       phase is never more than SEG-1 fp32 rotations away from an exact value
 //   4 * DM_BF_STAGE * 32 float2         per warp: A_v = kappa e^{-ik.v} of the patch's vertex slots for DM_BF_STAGE
 //                                       consecutive frequencies
-template <int MODE, int SEG>
+template <int MODE, int SEG, bool BAND>
 __global__ void __launch_bounds__(DM_BF_THREADS, DM_BF_MINCTA)
 dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__ vrec_g, DmPatchDev pt, int n_faces,
                    DmGridDev grid, int ix_begin, int ix_end, int rows_per_split, float tau_b,
@@ -251,7 +252,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         for (int iz = tid; iz < nzh; iz += DM_BF_THREADS) {
             const float kz = grid.kstep[2] * iz;
             float2 Gk = Grow[iz];
-            if (!dm_in_band(grid, nx, ny, iz)) Gk = make_float2(0.f, 0.f);  // narrow band: the cotangent outside is ignored
+            if (BAND && !dm_in_band(grid, nx, ny, iz)) Gk = make_float2(0.f, 0.f);  // narrow band: the cotangent outside is ignored
             float4 o;
             if (MODE == 1) {
                 o = make_float4(Gk.x, -Gk.y, kz, 0.f);                       // conj(G)
@@ -327,7 +328,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
 
         // narrow band: only the in-band interval of the row, started at a seed position
         int z_lo = 0, z_hi = nzh;
-        if (band_z != nullptr) {
+        if (BAND) {
             const int2 bz = band_z[ix * grid.ny + iy];
             z_lo = bz.x & ~(SEG - 1);
             z_hi = bz.y;
