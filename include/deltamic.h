@@ -90,7 +90,8 @@ typedef enum dm_option {
     DM_OPT_FORWARD_PATH  = 0, /* 0 = fast strip kernel (default), 1 = robust per-triangle kernel                  */
     DM_OPT_BACKWARD_PATH = 1, /* 0 = fast kernel (default), 1 = robust kernel                                     */
     DM_OPT_TAU           = 2, /* forward: gap-product threshold |pqr| below which a pair leaves the fast path       */
-    DM_OPT_TAU_BWD       = 3, /* backward: threshold on min|gap| * |pqr| below which a pair leaves the fast path      */
+    DM_OPT_TAU_BWD       = 3, /* backward: threshold on m1^2 m2 (the two smallest |gaps|) below which a pair leaves
+                                 the fast path                                                                     */
     DM_OPT_AREA_NORMALISED = 4 /* DM_SURFACE only; 1 = the paper's membrane density u = F / |Lambda| (PAPER.md:177-186
                                   eq. 12) and its gradient (eq. 13): forward divides by the total area, backward takes
                                   dL/du and adds the -(sum_k Re(conj(G) u)/|Lambda|) d|Lambda|/dv term (it recomputes

@@ -57,7 +57,7 @@ struct dm_plan {
     double* psfg_part = nullptr;     // [DM_PSFG_BLOCKS*6] block sums of the PSF gradient
     float* psfg_out = nullptr;       // [6] device result of the PSF gradient
     int fwd_path = 0, bwd_path = 0;  // 0 = fast, 1 = robust
-    float tau = 1e-2f, tau_b = 2e-4f;
+    float tau = 1e-2f, tau_b = 1.2e-4f;
     cufftHandle fft_xy = 0, fft_z = 0, fft_r2c = 0;
     bool have_xy = false, have_z = false, have_r2c = false, have_fft = false;
     // stage timing

@@ -30,7 +30,7 @@
 // row-independent table of exact z-phases kept in shared memory.
 //
 // Near-degenerate pairs (reading R4).  The derivative coefficients grow like 1/(gap^2 gap'), so a pair
-// with  min|gap| * |pqr| < tau_b  is excluded from the fast sums (its reciprocal is forced to 0) and flagged in a per-
+// with  m1^2 m2 <= tau_b  (m1 <= m2 the two smallest |gaps|)  is excluded from the fast sums (its reciprocal is forced to 0) and flagged in a per-
 // thread bit mask.  After each chunk of <= DM_BF_CHUNK frequencies the WARP pools its flagged pairs in shared memory,
 // sorted by owner, and evaluates them 32 at a time, one pair per lane whatever its owner: the series branch where all
 // gaps are small, the branch-free far-pair variant otherwise.  A segmented warp scan sums the results of one owner and
@@ -161,8 +161,11 @@ __device__ __forceinline__ bool dm_bf_pair(const float kz, const cf A0, const cf
 {
     const float p = fmaf(kz, ebz, prow), q = fmaf(kz, ecz, qrow), r = q - p;
     const float pqr = (p * q) * r;
+    // the largest derivative coefficient is 1/(m1^2 m2), m1 <= m2 <= m3 the sorted |gaps| (m3 = m1 + m2 always): the pair
+    // leaves the fast path when m1^2 m2 = m1 |pqr| / m3 <= tau_b  (also catches p = q = r = 0)
     const float m1 = fminf(fminf(fabsf(p), fabsf(q)), fabsf(r));
-    const bool bad = m1 * fabsf(pqr) < tau_b;
+    const float m3 = fmaxf(fmaxf(fabsf(p), fabsf(q)), fabsf(r));
+    const bool bad = !(m1 * fabsf(pqr) > tau_b * m3);
     const float R = bad ? 0.f : dm_rcp_approx(pqr);
     const float c0 = -r * R, c1 = q * R, c2 = -p * R;
     const float c0s = c0 * c0, c1s = c1 * c1, c2s = c2 * c2;
