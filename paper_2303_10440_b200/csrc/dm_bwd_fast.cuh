@@ -91,7 +91,8 @@ __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int3
         }
         const float eb[3] = {v[1][0] - v[0][0], v[1][1] - v[0][1], v[1][2] - v[0][2]};
         const float ec[3] = {v[2][0] - v[0][0], v[2][1] - v[0][1], v[2][2] - v[0][2]};
-        const float m[3] = {eb[1] * ec[2] - eb[2] * ec[1], eb[2] * ec[0] - eb[0] * ec[2], eb[0] * ec[1] - eb[1] * ec[0]};
+        float m[3];
+        dm_cross(eb, ec, m);
         const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
         float4* o = trec + (size_t)DM_BF_TREC * i;
         o[0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), __uint_as_float(pt.loc[i]));

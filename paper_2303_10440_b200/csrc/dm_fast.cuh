@@ -79,7 +79,8 @@ __global__ void dm_k_strip_geometry(const float* __restrict__ vertices, const in
                 a[d] = vertices[3 * i2 + d] - vertices[3 * i1 + d];
                 b[d] = vertices[3 * i3 + d] - vertices[3 * i1 + d];
             }
-            const float m[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+            float m[3];
+            dm_cross(a, b, m);
             if (mode == 1) r2.x = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
             else r2 = make_float4(m[0], m[1], m[2], 0.f);
             // longest edge of the triangle (squared)

@@ -51,7 +51,8 @@ __global__ void dm_k_geometry(const float* __restrict__ vertices, const int32_t*
     }
     const float eb[3] = {v2[0] - v1[0], v2[1] - v1[1], v2[2] - v1[2]};
     const float ec[3] = {v3[0] - v1[0], v3[1] - v1[1], v3[2] - v1[2]};
-    const float m[3] = {eb[1] * ec[2] - eb[2] * ec[1], eb[2] * ec[0] - eb[0] * ec[2], eb[0] * ec[1] - eb[1] * ec[0]};
+    float m[3];
+    dm_cross(eb, ec, m);
     const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
     rec[4 * (size_t)t + 0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), mn);
     rec[4 * (size_t)t + 1] = make_float4(eb[0], eb[1], eb[2], 0.f);
@@ -282,8 +283,9 @@ __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int3
     for (int p = 0; p < 3; ++p)
 #pragma unroll
         for (int d = 0; d < 3; ++d) e[p][d] = v[(p + 2) % 3][d] - v[(p + 1) % 3][d];
-    const float m[3] = {e[2][1] * e[0][2] - e[2][2] * e[0][1], e[2][2] * e[0][0] - e[2][0] * e[0][2],
-                        e[2][0] * e[0][1] - e[2][1] * e[0][0]};  // e_3 x e_1 = m_T
+    const float ecv[3] = {-e[1][0], -e[1][1], -e[1][2]};   // v_3 - v_1
+    float m[3];
+    dm_cross(e[2], ecv, m);                                // (v_2 - v_1) x (v_3 - v_1) = m_T, as in the geometry pre-pass
     const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
     float V[3][3];
 #pragma unroll

@@ -31,6 +31,24 @@ __device__ __forceinline__ cf cadd(cf a, cf b) { return {a.re + b.re, a.im + b.i
 __device__ __forceinline__ cf csub(cf a, cf b) { return {a.re - b.re, a.im - b.im}; }
 __device__ __forceinline__ cf cmul_i(cf a) { return {-a.im, a.re}; }  // i * a
 
+// a b - c d with one rounding error of the result's own size (Kahan): exactly 0 when the two products are equal, so a
+// triangle whose fp32 vertices are exactly collinear gets m_T = 0 exactly, as in the fp64 oracle (reading R19), and the
+// normal of a thin triangle is as accurate as its fp32 edges allow.
+__device__ __forceinline__ float dm_dop(float a, float b, float c, float d)
+{
+    const float w = __fmul_rn(c, d);
+    const float e = __fmaf_rn(-c, d, w);
+    const float f = __fmaf_rn(a, b, -w);
+    return __fadd_rn(f, e);
+}
+// m = a x b
+__device__ __forceinline__ void dm_cross(const float a[3], const float b[3], float m[3])
+{
+    m[0] = dm_dop(a[1], b[2], a[2], b[1]);
+    m[1] = dm_dop(a[2], b[0], a[0], b[2]);
+    m[2] = dm_dop(a[0], b[1], a[1], b[0]);
+}
+
 // sinc(h) = sin(h)/h and dsinc(h) = d/dh sinc = (cos h - sinc h)/h, without cancellation near 0.
 __device__ __forceinline__ void dm_sinc_dsinc(float h, float& s, float& ds)
 {

@@ -305,3 +305,36 @@ def test_area_normalised_density_eq12_eq13(dm):
     plan.close()
     with pytest.raises(dm.DeltamicError):             # volume mode has no area normalisation
         _plan(dm, w, 0).set_option(dm.DM_OPT_AREA_NORMALISED, 1)
+
+
+def test_degenerate_and_non_manifold_meshes_surface_mode(dm):
+    """Edge cases of the input (readings R19, R20): a non-manifold "book" of four triangles on one edge, a zero-area
+    triangle, a face that repeats a vertex, an isolated vertex no face uses, a single-triangle mesh and the smallest
+    grid (2 x 2 x 2).  Surface mode is a plain sum over triangles, so the oracle defines every case; forward and
+    backward (box-exact degeneracies included: the book's spine lies on the z axis) must match it."""
+    import torch
+    v = np.array([[0, 0, -0.2], [0, 0, 0.2], [0.3, 0, 0], [0, 0.25, 0.05], [-0.2, -0.1, 0], [0.1, -0.3, 0.1],
+                  [0.05, 0.05, 0.05], [0.4, 0.4, 0.4]], dtype=np.float32)          # vertex 7 is used by no face
+    f = np.array([[0, 1, 2], [0, 1, 3], [1, 0, 4], [0, 1, 5],                      # four pages on the edge (0,1)
+                  [2, 6, 6],                                                        # repeated vertex (zero area)
+                  [2, 3, 2]], dtype=np.int32)                                       # repeated vertex again
+    vz = v.copy()
+    vz = np.vstack([vz, 0.5 * (vz[2] + vz[3])[None]])                               # vertex 8 = midpoint of (2,3)
+    fz = np.vstack([f, [[2, 8, 3]]]).astype(np.int32)                               # collinear: zero area, distinct vertices
+    cases = [(vz.astype(np.float32), fz, (12, 10, 8)), (v[:3].copy(), f[:1].copy(), (8, 8, 8)), (v[:3].copy(), f[:1].copy(), (2, 2, 2))]
+    for vv, ff, n in cases:
+        spacing = tuple(1.0 / x for x in n)
+        plan = dm.Plan(n, spacing, (0, 0, 0), 1, torch.as_tensor(ff, device="cuda"), vv.shape[0])
+        F = plan.mesh_ft_forward(_dev(vv)).cpu().numpy()
+        ref = oracle.mesh_ft_forward_grid(vv, ff, n, spacing, 1)
+        assert np.isfinite(F.view(np.float32)).all()
+        assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0])
+        rng = np.random.default_rng(17)
+        G = (rng.standard_normal(ref.shape) + 1j * rng.standard_normal(ref.shape)).astype(np.complex64)
+        dv = plan.mesh_ft_backward(_dev(vv), _dev(G)).cpu().numpy()
+        dref = oracle.mesh_ft_backward_grid(vv, ff, n, spacing, 1, G.astype(np.complex128))
+        assert np.isfinite(dv).all()
+        assert _rel_l2(dv, dref) <= GRAD_TOL, (n, _rel_l2(dv, dref))
+        unused = sorted(set(range(vv.shape[0])) - set(ff.reshape(-1).tolist()))
+        assert (dv[unused] == 0).all()                                              # no face, no gradient
+        plan.close()
