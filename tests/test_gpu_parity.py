@@ -338,3 +338,31 @@ def test_degenerate_and_non_manifold_meshes_surface_mode(dm):
         unused = sorted(set(range(vv.shape[0])) - set(ff.reshape(-1).tolist()))
         assert (dv[unused] == 0).all()                                              # no face, no gradient
         plan.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_odd_grid_sizes_and_non_unit_box(dm, mode):
+    """Odd N_x, N_y (no Nyquist rows), a box that is not the unit cube and a mesh that is not centred: forward, backward
+    and render against the oracle on the full grid."""
+    import torch
+    n = (15, 9, 10)
+    spacing = (0.07, 0.11, 0.13)
+    origin = (-0.4, -0.5, -0.6)
+    v, f = icosphere(2, 0.31, (0.05, -0.04, 0.02))
+    v = v.astype(np.float32)
+    plan = dm.Plan(n, spacing, origin, mode, torch.as_tensor(f, device="cuda"), v.shape[0])
+    F = plan.mesh_ft_forward(_dev(v)).cpu().numpy()
+    ref = oracle.mesh_ft_forward_grid(v, f, n, spacing, mode)
+    assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0])
+    rng = np.random.default_rng(23)
+    G = (rng.standard_normal(ref.shape) + 1j * rng.standard_normal(ref.shape)).astype(np.complex64)
+    dv = plan.mesh_ft_backward(_dev(v), _dev(G)).cpu().numpy()
+    assert _rel_l2(dv, oracle.mesh_ft_backward_grid(v, f, n, spacing, mode, G.astype(np.complex128))) <= GRAD_TOL
+    cov = np.array([0.012, 0.02, 0.03, 0.002, -0.004, 0.003])
+    img = plan.render(_dev(v), cov).cpu().numpy()
+    iref = oracle.render(v, f, n, spacing, origin, cov, mode)
+    assert np.abs(img - iref).max() <= IMG_TOL * np.abs(iref).max()
+    y = rng.standard_normal(n).astype(np.float32)
+    dvr = plan.render_backward(_dev(v), cov, _dev(y)).cpu().numpy()
+    assert _rel_l2(dvr, oracle.render_backward(v, f, n, spacing, origin, cov, mode, y.astype(np.float64))) <= GRAD_TOL
+    plan.close()
