@@ -19,6 +19,8 @@ from .mesh_ft import (  # noqa: F401
     mesh_ft_backward,
     mesh_ft_backward_grid,
     mesh_ft_backward_normalised,
+    mesh_ft_backward_weighted,
+    mesh_ft_forward_weighted,
     mesh_ft_forward_normalised,
     surface_area_and_gradient,
     num_threads,

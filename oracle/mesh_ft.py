@@ -168,3 +168,30 @@ def mesh_ft_backward_normalised(vertices, faces, kvec, G) -> np.ndarray:
     u = mesh_ft_forward(vertices, faces, kvec, 1) / area
     s = float((np.conj(Gc) * u).real.sum())
     return bare / area - (s / area) * darea
+
+
+# ---- per-face density weights ("a weighted sum of the FT of surfaces with different densities") -------------
+def _weight_groups(faces, weights):
+    f = np.asarray(faces, dtype=np.int32).reshape(-1, 3)
+    w = np.asarray(weights, dtype=np.float64).reshape(-1)
+    if w.shape[0] != f.shape[0]:
+        raise ValueError("one weight per face")
+    return [(float(u), f[w == u]) for u in np.unique(w)]
+
+
+def mesh_ft_forward_weighted(vertices, faces, kvec, mode: int, weights) -> np.ndarray:
+    """F(k) = sum_T w_T (triangle term of T): by linearity, the sum over the groups of equal weight of w times the FT of
+    the group's faces.  Meant for a few distinct weights (one per surface), as in the paper."""
+    k = np.asarray(kvec, dtype=np.float64).reshape(-1, 3)
+    out = np.zeros(k.shape[0], dtype=np.complex128)
+    for u, fg in _weight_groups(faces, weights):
+        out += u * mesh_ft_forward(vertices, fg, k, mode)
+    return out
+
+
+def mesh_ft_backward_weighted(vertices, faces, kvec, mode: int, G, weights) -> np.ndarray:
+    v = np.asarray(vertices, dtype=np.float64).reshape(-1, 3)
+    out = np.zeros_like(v)
+    for u, fg in _weight_groups(faces, weights):
+        out += u * mesh_ft_backward(vertices, fg, kvec, mode, G)
+    return out

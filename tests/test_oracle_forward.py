@@ -170,3 +170,23 @@ def test_empty_mesh_and_empty_frequency_list():
     assert oracle.mesh_ft_forward(v, f, np.zeros((0, 3)), VOL).shape == (0,)
     F = oracle.mesh_ft_forward(v, np.zeros((0, 3), np.int32), np.ones((3, 3)), SURF)
     assert np.all(F == 0)
+
+
+def test_per_face_weights_are_linear_in_the_density():
+    """PAPER.md:127 (reading R23): two nested closed surfaces with densities 1 and 0.5 in volume mode give the FT of
+    a ball of density 1 minus half a ball -- i.e. F_outer - 0.5 F_inner with the inner sphere's faces weighted -0.5 --
+    and F(0) is the weighted volume; in surface mode the weights scale each membrane's area."""
+    from workloads import icosphere
+    vo, fo = icosphere(2, 0.4)
+    vi, fi = icosphere(1, 0.2, (0.03, 0.0, -0.02))
+    v = np.vstack([vo, vi])
+    f = np.vstack([fo, fi + len(vo)]).astype(np.int32)
+    w = np.concatenate([np.ones(len(fo)), -0.5 * np.ones(len(fi))])
+    k = np.random.default_rng(4).uniform(-30, 30, size=(25, 3))
+    k[0] = 0
+    for mode in (VOL, SURF):
+        got = oracle.mesh_ft_forward_weighted(v, f, k, mode, w)
+        want = oracle.mesh_ft_forward(vo, fo, k, mode) - 0.5 * oracle.mesh_ft_forward(vi, fi, k, mode)
+        assert np.abs(got - want).max() <= 1e-13 * abs(want[0])
+    vol = lambda vv, ff: np.einsum("ij,ij->i", vv[ff[:, 0]], np.cross(vv[ff[:, 1]], vv[ff[:, 2]])).sum() / 6.0
+    assert abs(oracle.mesh_ft_forward_weighted(v, f, k[:1], VOL, w)[0] - (vol(vo, fo) - 0.5 * vol(vi, fi))) < 1e-14
