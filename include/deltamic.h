@@ -76,6 +76,13 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
  * DESIGN.md section 9).  Default: the whole grid.  dm_render* require the whole grid. */
 int dm_plan_set_slab(dm_plan* plan, int32_t ix_begin, int32_t ix_end);
 
+/* Per-face density weights (the density is "a weighted sum" over surfaces of different fluorophore
+ * concentration).  weights_dev = device float32 [n_faces], copied here (the caller may free it); every triangle term of
+ * F, and so of the gradients, is multiplied by its face's weight: DM_SURFACE sum_T w_T int_T e^{-ik.x} dS, DM_VOLUME
+ * (i/|k|^2) sum_T w_T (k.m_T) f_T (closed components with one weight each are regions of that density; negative weights
+ * carve holes).  F(0) is the weighted area / volume.  NULL switches the weights off (all 1, the default). */
+int dm_plan_set_face_weights(dm_plan* plan, const float* weights_dev);
+
 /* Narrow band ("evaluate the FT only where the PSF spectrum is above 1 % of its maximum").
  * With psf_cov_host = 6 floats on the HOST (covariance B of a Gaussian PSF, order xx, yy, zz, xy, xz, yz) and
  * 0 < cutoff < 1, the mesh-FT calls of this plan evaluate only the stored frequencies with

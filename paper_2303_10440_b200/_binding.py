@@ -12,7 +12,7 @@ DM_OPT_FORWARD_PATH, DM_OPT_BACKWARD_PATH, DM_OPT_TAU, DM_OPT_TAU_BWD, DM_OPT_AR
 
 # every symbol include/deltamic.h declares
 _SYMBOLS = (
-    "dm_plan_create", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_render",
+    "dm_plan_create", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_render",
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
     "dm_plan_launch_count", "dm_plan_destroy", "dm_error_string", "dm_version",
 )
@@ -54,6 +54,7 @@ def load_library():
                                    ctypes.c_int32, ip, vp]
     lib.dm_plan_set_slab.argtypes = [vp, ctypes.c_int32, ctypes.c_int32]
     lib.dm_plan_set_option.argtypes = [vp, ctypes.c_int, ctypes.c_double]
+    lib.dm_plan_set_face_weights.argtypes = [vp, fp]
     lib.dm_plan_set_narrow_band.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_float]
     lib.dm_mesh_ft_forward.argtypes = [vp, fp, fp]
     lib.dm_mesh_ft_backward.argtypes = [vp, fp, fp, fp]
@@ -154,6 +155,11 @@ class Plan:
     # -- the C ABI, one method per entry point ------------------------------------------------------------------
     def set_slab(self, ix_begin: int, ix_end: int):
         _check(self._lib.dm_plan_set_slab(self._h, int(ix_begin), int(ix_end)), "dm_plan_set_slab")
+
+    def set_face_weights(self, weights=None):
+        """Per-face density weights (float32 CUDA tensor [n_faces]); ``None`` = all 1."""
+        ptr = None if weights is None else self._f32(weights, self.n_faces, "face weights").data_ptr()
+        _check(self._lib.dm_plan_set_face_weights(self._h, ptr), "dm_plan_set_face_weights")
 
     def set_narrow_band(self, psf_cov=None, cutoff: float = 0.01):
         """Evaluate only the frequencies with exp(-1/2 k^T B k) > cutoff; ``psf_cov=None`` = off."""

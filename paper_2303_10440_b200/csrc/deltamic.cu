@@ -51,6 +51,7 @@ struct dm_plan {
     bool normalise = false;          // DM_OPT_AREA_NORMALISED (surface mode): u = F/|Lambda|, eq. 12-13
     double* dc_total = nullptr;      // [1] fp64 volume / total area of the last forward (k = 0 kernels)
     double* dot_part = nullptr;      // [DM_DOT_BLOCKS + 1] block sums and result of sum_k Re(conj(G) F)
+    float* face_w = nullptr;         // [n_faces] per-face density weights, valid while gd.face_w points at it
     int2* band_z = nullptr;          // [nx*ny] in-band z interval of every row (narrow band), valid while band_on
     bool band_on = false;
     float2* spec3 = nullptr;         // [n_k] forward spectrum recomputed for the PSF gradient (allocated on first use)
@@ -213,7 +214,7 @@ int run_forward_raw(dm_plan* p, const float* vertices_dev, float* F_dev)
     int rc = p->fwd_path == 0 ? run_forward_fast(p, vertices_dev, F_dev) : run_forward_robust(p, vertices_dev, F_dev);
     if (rc) return rc;
     if (p->ix_begin == 0) {
-        dm_k_dc_partial<<<DM_DC_BLOCKS, 256, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode, p->dc_part);
+        dm_k_dc_partial<<<DM_DC_BLOCKS, 256, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode, p->gd.face_w, p->dc_part);
         if ((rc = check_launch(p))) return rc;
         dm_k_dc_final<<<1, DM_DC_BLOCKS, 0, p->stream>>>(p->dc_part, F_dev, p->dc_total);
         rc = check_launch(p);
@@ -300,7 +301,8 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     stage_begin(p, 3);
     dm_k_corner_grads<<<(p->n_faces + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode,
                                                                        n_split, p->part, (const float2*)G_dev,
-                                                                       p->ix_begin == 0 ? 1 : 0, area_total, sdot, p->corner);
+                                                                       p->ix_begin == 0 ? 1 : 0, area_total, sdot, p->gd.face_w,
+                                                                       p->corner);
     rc = check_launch(p);
     if (rc) return rc;
     dm_k_vertex_gather<<<(p->n_vertices + 127) / 128, 128, 0, p->stream>>>(p->csr_off, p->csr_corner, p->n_vertices,
@@ -387,6 +389,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
     for (int i = 0; i < 6; ++i) p->gd.band_cov[i] = 0.f;
     p->gd.band_lim = INFINITY;
     p->gd.nzb = p->gd.nzh;
+    p->gd.face_w = nullptr;
     p->ix_begin = 0;
     p->ix_end = p->gd.nx;
     // gap-product threshold of the forward fast path: one excluded-or-not pair may cost ~1e-6 (sum|d|)/tau of ONE
@@ -503,6 +506,21 @@ int dm_plan_set_slab(dm_plan* p, int32_t ix_begin, int32_t ix_end)
     if (!p || ix_begin < 0 || ix_end > p->gd.nx || ix_begin >= ix_end) return DM_ERR_INVALID_ARG;
     p->ix_begin = ix_begin;
     p->ix_end = ix_end;
+    return DM_OK;
+}
+
+int dm_plan_set_face_weights(dm_plan* p, const float* weights_dev)
+{
+    if (!p) return DM_ERR_INVALID_ARG;
+    if (!weights_dev) {
+        p->gd.face_w = nullptr;
+        return DM_OK;
+    }
+    if (!p->face_w && cudaMalloc(&p->face_w, (size_t)p->n_faces * sizeof(float)) != cudaSuccess) return DM_ERR_ALLOC;
+    if (cudaMemcpyAsync(p->face_w, weights_dev, (size_t)p->n_faces * sizeof(float), cudaMemcpyDeviceToDevice, p->stream) !=
+        cudaSuccess)
+        return DM_ERR_CUDA;
+    p->gd.face_w = p->face_w;
     return DM_OK;
 }
 
@@ -702,6 +720,7 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->dc_part);
     cudaFree(p->dc_total);
     cudaFree(p->dot_part);
+    cudaFree(p->face_w);
     cudaFree(p->band_z);
     cudaFree(p->spec3);
     cudaFree(p->psfg_part);

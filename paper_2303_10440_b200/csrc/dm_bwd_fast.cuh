@@ -93,7 +93,9 @@ __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int3
         const float ec[3] = {v[2][0] - v[0][0], v[2][1] - v[0][1], v[2][2] - v[0][2]};
         float m[3];
         dm_cross(eb, ec, m);
-        const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+        const float wf = grid.face_w ? grid.face_w[f] : 1.0f;   // density weight of the face
+        const float mn = wf * sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+        m[0] *= wf, m[1] *= wf, m[2] *= wf;
         float4* o = trec + (size_t)DM_BF_TREC * i;
         o[0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), __uint_as_float(pt.loc[i]));
         o[1] = make_float4(eb[0], eb[1], eb[2], 0.f);

@@ -81,8 +81,9 @@ __global__ void dm_k_strip_geometry(const float* __restrict__ vertices, const in
             }
             float m[3];
             dm_cross(a, b, m);
-            if (mode == 1) r2.x = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
-            else r2 = make_float4(m[0], m[1], m[2], 0.f);
+            const float wf = grid.face_w ? grid.face_w[f] : 1.0f;   // density weight of the face
+            if (mode == 1) r2.x = wf * sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+            else r2 = make_float4(wf * m[0], wf * m[1], wf * m[2], 0.f);
             // longest edge of the triangle (squared)
             const float c[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]};
             h2 = fmaxf(fmaxf(a[0] * a[0] + a[1] * a[1] + a[2] * a[2], b[0] * b[0] + b[1] * b[1] + b[2] * b[2]),

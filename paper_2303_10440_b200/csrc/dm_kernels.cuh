@@ -19,6 +19,7 @@ struct DmGridDev {
     // the Gaussian PSF of covariance B, band_lim = ln(1/cutoff)); band_lim = +inf switches the band off
     float band_cov[6];        // xx yy zz xy xz yz
     float band_lim;
+    const float* face_w;      // per-face density weights, device [n_faces]; nullptr = all 1
     int nzb;                  // stored z-frequencies 0..nzb-1 can be inside the band (nzb = nzh when the band is off)
 };
 
@@ -53,7 +54,9 @@ __global__ void dm_k_geometry(const float* __restrict__ vertices, const int32_t*
     const float ec[3] = {v3[0] - v1[0], v3[1] - v1[1], v3[2] - v1[2]};
     float m[3];
     dm_cross(eb, ec, m);
-    const float mn = sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+    const float wf = grid.face_w ? grid.face_w[t] : 1.0f;   // density weight of the face: scales m_T and |m_T|
+    const float mn = wf * sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+    m[0] *= wf, m[1] *= wf, m[2] *= wf;
     rec[4 * (size_t)t + 0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), mn);
     rec[4 * (size_t)t + 1] = make_float4(eb[0], eb[1], eb[2], 0.f);
     rec[4 * (size_t)t + 2] = make_float4(ec[0], ec[1], ec[2], 0.f);
@@ -65,7 +68,7 @@ __global__ void dm_k_geometry(const float* __restrict__ vertices, const int32_t*
 #define DM_DC_BLOCKS 64
 __global__ void __launch_bounds__(256)
 dm_k_dc_partial(const float* __restrict__ vertices, const int32_t* __restrict__ faces, int n_faces, int mode,
-                double* __restrict__ partial)
+                const float* __restrict__ face_w, double* __restrict__ partial)
 {
     __shared__ double sh[256];
     double acc = 0.0;
@@ -74,13 +77,14 @@ dm_k_dc_partial(const float* __restrict__ vertices, const int32_t* __restrict__ 
         const double a[3] = {vertices[3 * i1], vertices[3 * i1 + 1], vertices[3 * i1 + 2]};
         const double b[3] = {vertices[3 * i2], vertices[3 * i2 + 1], vertices[3 * i2 + 2]};
         const double c[3] = {vertices[3 * i3], vertices[3 * i3 + 1], vertices[3 * i3 + 2]};
+        const double wf = face_w ? (double)face_w[t] : 1.0;
         if (mode == 0) {
-            acc += (a[0] * (b[1] * c[2] - b[2] * c[1]) + a[1] * (b[2] * c[0] - b[0] * c[2]) +
+            acc += wf * (a[0] * (b[1] * c[2] - b[2] * c[1]) + a[1] * (b[2] * c[0] - b[0] * c[2]) +
                     a[2] * (b[0] * c[1] - b[1] * c[0])) * (1.0 / 6.0);
         } else {
             const double e[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]}, f[3] = {c[0] - a[0], c[1] - a[1], c[2] - a[2]};
             const double m[3] = {e[1] * f[2] - e[2] * f[1], e[2] * f[0] - e[0] * f[2], e[0] * f[1] - e[1] * f[0]};
-            acc += 0.5 * sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+            acc += wf * 0.5 * sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
         }
     }
     sh[threadIdx.x] = acc;
@@ -253,7 +257,8 @@ dm_k_backward_robust(const float4* __restrict__ rec, int n_faces, DmGridDev grid
 __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int32_t* __restrict__ faces, int n_faces,
                                   int mode, int n_split, const float* __restrict__ part,
                                   const float2* __restrict__ G, int has_dc, const double* __restrict__ area_total,
-                                  const double* __restrict__ sdot, float* __restrict__ corner)
+                                  const double* __restrict__ sdot, const float* __restrict__ face_w,
+                                  float* __restrict__ corner)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n_faces) return;
@@ -294,6 +299,7 @@ __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int3
         V[2][d] = s[10 + d];
         V[0][d] = s[4 + d] - s[7 + d] - s[10 + d];
     }
+    const float wf = face_w ? face_w[t] : 1.0f;   // density weight of the face
     float grad[3][3];
     if (mode == 1) {
         const float inv = (mn >= 1e-30f) ? 1.0f / mn : 0.f;
@@ -303,7 +309,7 @@ __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int3
             const float w[3] = {e[p][1] * N[2] - e[p][2] * N[1], e[p][2] * N[0] - e[p][0] * N[2],
                                 e[p][0] * N[1] - e[p][1] * N[0]};
 #pragma unroll
-            for (int d = 0; d < 3; ++d) grad[p][d] = (mn >= 1e-30f) ? fmaf(mn, V[p][d], -w[d] * s[0]) : 0.f;
+            for (int d = 0; d < 3; ++d) grad[p][d] = (mn >= 1e-30f) ? wf * fmaf(mn, V[p][d], -w[d] * s[0]) : 0.f;
         }
     } else {
         const float Q[3] = {s[1], s[2], s[3]};
@@ -317,7 +323,7 @@ __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int3
             const float x[3] = {Q[1] * e[p][2] - Q[2] * e[p][1], Q[2] * e[p][0] - Q[0] * e[p][2],
                                 Q[0] * e[p][1] - Q[1] * e[p][0]};
 #pragma unroll
-            for (int d = 0; d < 3; ++d) grad[p][d] = x[d] + V[p][d] + g0 * c[d];
+            for (int d = 0; d < 3; ++d) grad[p][d] = wf * (x[d] + g0 * c[d]) + V[p][d];   // V carries w_T through k.m_T
         }
     }
 #pragma unroll

@@ -366,3 +366,33 @@ def test_odd_grid_sizes_and_non_unit_box(dm, mode):
     dvr = plan.render_backward(_dev(v), cov, _dev(y)).cpu().numpy()
     assert _rel_l2(dvr, oracle.render_backward(v, f, n, spacing, origin, cov, mode, y.astype(np.float64))) <= GRAD_TOL
     plan.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_per_face_density_weights(dm, mode):
+    """PAPER.md:127 (reading R23): two nested surfaces with weights 1 and -0.5 (a shell of density 1 around a core of
+    density 0.5 in volume mode): forward and backward of the fast and the robust kernels against the oracle."""
+    import torch
+    vo, fo = icosphere(2, 0.4)
+    vi, fi = icosphere(2, 0.2, (0.03, 0.0, -0.02))
+    v = np.vstack([vo, vi]).astype(np.float32)
+    f = np.vstack([fo, fi + len(vo)]).astype(np.int32)
+    wts = np.concatenate([np.ones(len(fo)), -0.5 * np.ones(len(fi))]).astype(np.float32)
+    n, spacing = (16, 20, 12), (1 / 16, 1 / 20, 1 / 12)
+    k = oracle.frequency_grid(n, spacing).reshape(-1, 3)
+    plan = dm.Plan(n, spacing, (0, 0, 0), mode, torch.as_tensor(f, device="cuda"), v.shape[0])
+    plan.set_face_weights(_dev(wts))
+    ref = oracle.mesh_ft_forward_weighted(v, f, k, mode, wts)
+    G = spectrum_cotangent(build_workload(1, grid_override=n))
+    dref = oracle.mesh_ft_backward_weighted(v, f, k, mode, G.reshape(-1).astype(np.complex128), wts)
+    for path in (0, 1):
+        plan.set_option(dm.DM_OPT_FORWARD_PATH, path)
+        plan.set_option(dm.DM_OPT_BACKWARD_PATH, path)
+        F = plan.mesh_ft_forward(_dev(v)).cpu().numpy().reshape(-1)
+        assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0]), path
+        dv = plan.mesh_ft_backward(_dev(v), _dev(G)).cpu().numpy()
+        assert _rel_l2(dv, dref) <= GRAD_TOL, path
+    plan.set_face_weights(None)
+    F1 = plan.mesh_ft_forward(_dev(v)).cpu().numpy().reshape(-1)
+    assert np.abs(F1 - oracle.mesh_ft_forward(v, f, k, mode)).max() <= FWD_TOL * abs(ref[0])
+    plan.close()
