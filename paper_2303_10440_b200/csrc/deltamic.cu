@@ -441,7 +441,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
             const long long kblocks = ((long long)p->gd.nx * n_yruns * p->gd.nzh + DM_FAST_THREADS - 1) / DM_FAST_THREADS;
             const long long slots = (long long)p->n_sm * 4;
             long long want = (6 * slots + kblocks - 1) / kblocks;
-            want = std::min<long long>(want, std::max<long long>(1, n_faces / 1536));
+            want = std::min<long long>(want, std::max<long long>(1, n_faces / 384));   // at least one tile of strip records per chunk
             want = std::max<long long>(1, std::min<long long>(want, 64));
             DmStripRecords sr;
             try { sr = dm_build_strips(faces_h.data(), n_faces, n_vertices, (int)want); } catch (...) { rc = DM_ERR_ALLOC; break; }
