@@ -3,7 +3,7 @@
  * (arxiv 2303.10440, "Differentiable Rendering for 3D Fluorescence Microscopy").
  *
  * Citations are "PAPER.md:<line>" of the paper text plus the equation they fall in; "north_star" is
- * BASELINE.json's statement of the build.  Readings R1..R24 are listed in DESIGN.md section 3.
+ * BASELINE.json's statement of the build.  Readings R1..R25 are listed in DESIGN.md section 3.
  *
  * The library renders a triangle mesh into a 3D image through the Fourier domain (Fig. 1,
  * :83-89 eq. 1-2):   image = irfft3( F . h_hat . e^{+i k.x0} ) / (h_x h_y h_z),

@@ -238,8 +238,8 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     int rps = 1;
     const int n_split = backward_splits(p, &rps);
     dim3 grid((p->n_faces + 127) / 128, n_split);
-    // seed spacing of the fast kernel: the smallest SEG whose seed table (ceil(nzh/SEG)-1 entries x 3 vertices x 128
-    // threads x 8 B) has at most 8 entries per vertex
+    // seed spacing of the fast kernel: the smallest SEG whose seed table (ceil(nzh/SEG)-1 entries x 128 threads x 8 B,
+    // one vertex slot per thread) has at most 8 entries per vertex
     const int nzh = p->gd.nzh;
 #if defined(DM_BF_FORCE_SEG)
     const int seg = DM_BF_FORCE_SEG;
