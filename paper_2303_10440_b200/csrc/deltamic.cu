@@ -102,11 +102,12 @@ void stage_reset(dm_plan* p)
 
 int backward_splits(const dm_plan* p, int* rows_per_split)
 {
-    // enough (triangle-block x k-split) CTAs to fill the machine (4 CTAs per SM) about 12 times over: short tail
+    // enough (triangle-block x k-split) CTAs to fill the machine (5 CTAs per SM) about 10 times over: short tail
     const int n_rows = (p->ix_end - p->ix_begin) * p->gd.ny;
     const int tri_blocks = (p->n_faces + 127) / 128;
     int want = (p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
-    if (p->band_on) want = p->n_split_max;   // rows differ in cost under the narrow band: many small CTAs balance the load
+    if (p->band_on) want = std::max(want, std::min(p->n_split_max, 64));   // rows differ in cost under the narrow band:
+                                                                             // many small CTAs balance the load
     if (want < 1) want = 1;
     if (want > n_rows) want = n_rows;
     if (want > p->n_split_max) want = p->n_split_max;
@@ -423,7 +424,14 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
         for (size_t i = 0; i < faces_h.size(); ++i) cor[(size_t)fill[faces_h[i]]++] = (int32_t)i;
 
         const size_t nk = n_k_of(p);
-        p->n_split_max = 64;
+        // k-splits of the backward: a small mesh has few triangle blocks, so it needs many splits to fill the machine
+        // (up to 48 CTAs per SM slot), within 64 M floats of partial sums
+        {
+            const long long tri_blocks = ((long long)n_faces + DM_BF_THREADS - 1) / DM_BF_THREADS;
+            long long m = ((long long)p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
+            m = std::min<long long>(m, (64LL << 20) / ((long long)DM_BWD_NSUM * n_faces));
+            p->n_split_max = (int)std::max<long long>(64, std::min<long long>(m, 4096));
+        }
         if (cudaMalloc(&p->faces, faces_h.size() * sizeof(int32_t)) != cudaSuccess ||
             cudaMalloc(&p->csr_off, off.size() * sizeof(int32_t)) != cudaSuccess ||
             cudaMalloc(&p->csr_corner, cor.size() * sizeof(int32_t)) != cudaSuccess ||
