@@ -88,7 +88,8 @@ int dm_plan_set_face_weights(dm_plan* plan, const float* weights_dev);
  * 0 < cutoff < 1, the mesh-FT calls of this plan evaluate only the stored frequencies with
  * exp(-1/2 k^T B k) > cutoff: dm_mesh_ft_forward writes 0 everywhere else, dm_mesh_ft_backward ignores dL/dF there
  * (the gradient of the banded forward).  dm_render* use the band too; B is normally the PSF they are called with.
- * psf_cov_host = NULL switches the band off (the default).  k = 0 is always inside the band. */
+ * psf_cov_host = NULL switches the band off (the default).  k = 0 is always inside the band.  Setting the band
+ * synchronises the stream (it builds the list of active frequencies). */
 int dm_plan_set_narrow_band(dm_plan* plan, const float* psf_cov_host, float cutoff);
 
 /* Tuning / debugging knobs.  Defaults are the product path; the "robust" paths evaluate EVERY pair through the

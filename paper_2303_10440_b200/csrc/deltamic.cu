@@ -52,6 +52,7 @@ struct dm_plan {
     double* dc_total = nullptr;      // [1] fp64 volume / total area of the last forward (k = 0 kernels)
     double* dot_part = nullptr;      // [DM_DOT_BLOCKS + 1] block sums and result of sum_k Re(conj(G) F)
     float* face_w = nullptr;         // [n_faces] per-face density weights, valid while gd.face_w points at it
+    uint32_t* band_slots = nullptr;  // the forward kernel's thread list under the narrow band
     int2* band_z = nullptr;          // [nx*ny] in-band z interval of every row (narrow band), valid while band_on
     bool band_on = false;
     float2* spec3 = nullptr;         // [n_k] forward spectrum recomputed for the PSF gradient (allocated on first use)
@@ -185,7 +186,8 @@ int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
     int rc = check_launch(p);
     if (rc) return rc;
     const int n_yruns = (p->gd.ny + DM_K - 1) / DM_K;
-    const long long n_thr = (long long)(p->ix_end - p->ix_begin) * n_yruns * p->gd.nzb;
+    const long long n_thr = p->gd.band_slots ? (long long)p->gd.n_band_slots
+                                             : (long long)(p->ix_end - p->ix_begin) * n_yruns * p->gd.nzh;
     dim3 grid((unsigned)((n_thr + DM_FAST_THREADS - 1) / DM_FAST_THREADS), (unsigned)p->st_n_chunks);
     const size_t stride = n_k_of(p);
     if (p->mode == DM_SURFACE)
@@ -390,6 +392,8 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
     for (int i = 0; i < 6; ++i) p->gd.band_cov[i] = 0.f;
     p->gd.band_lim = INFINITY;
     p->gd.nzb = p->gd.nzh;
+    p->gd.band_slots = nullptr;
+    p->gd.n_band_slots = 0;
     p->gd.face_w = nullptr;
     p->ix_begin = 0;
     p->ix_end = p->gd.nx;
@@ -539,6 +543,8 @@ int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
         p->band_on = false;
         p->gd.band_lim = INFINITY;
         p->gd.nzb = p->gd.nzh;
+        p->gd.band_slots = nullptr;
+        p->gd.n_band_slots = 0;
         return DM_OK;
     }
     if (!(cutoff > 0.f) || !(cutoff < 1.f)) return DM_ERR_INVALID_ARG;
@@ -563,8 +569,51 @@ int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
         }
     }
     const int n_rows = p->gd.nx * p->gd.ny;
+    p->gd.band_slots = nullptr;   // the row intervals are computed with the band test alone
+    p->gd.n_band_slots = 0;
     dm_k_band_rows<<<(n_rows + 127) / 128, 128, 0, p->stream>>>(p->gd, p->band_z);
-    return check_launch(p);
+    int rc = check_launch(p);
+    if (rc) return rc;
+    // the forward kernel's thread list: every (i_x, run of DM_K signed y-frequencies, i_z) with a frequency in the band
+    std::vector<int2> bz;
+    std::vector<uint32_t> slots;
+    try {
+        bz.resize((size_t)n_rows);
+    } catch (...) { return DM_ERR_ALLOC; }
+    if (cudaMemcpyAsync(bz.data(), p->band_z, (size_t)n_rows * sizeof(int2), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+        cudaStreamSynchronize(p->stream) != cudaSuccess)
+        return DM_ERR_CUDA;
+    const int ny = p->gd.ny, n_yruns = (ny + DM_K - 1) / DM_K;
+    if (p->gd.nx <= 4096 && n_yruns <= 2048 && p->gd.nzh <= 512) {
+        try {
+            for (int ix = 0; ix < p->gd.nx; ++ix)
+                for (int yrun = 0; yrun < n_yruns; ++yrun) {
+                    int lo = p->gd.nzh, hi = 0;
+                    for (int j = 0; j < DM_K; ++j) {
+                        const int nys = -(ny / 2) + yrun * DM_K + j;
+                        if (nys > (ny - 1) / 2) break;
+                        const int2 b = bz[(size_t)ix * ny + (nys < 0 ? nys + ny : nys)];
+                        if (b.y > b.x) {
+                            lo = std::min(lo, b.x);
+                            hi = std::max(hi, b.y);
+                        }
+                    }
+                    for (int iz = lo; iz < hi; ++iz) slots.push_back(((uint32_t)ix << 20) | ((uint32_t)yrun << 9) | (uint32_t)iz);
+                }
+        } catch (...) { return DM_ERR_ALLOC; }
+        if (!slots.empty()) {
+            cudaFree(p->band_slots);
+            p->band_slots = nullptr;
+            if (cudaMalloc(&p->band_slots, slots.size() * sizeof(uint32_t)) != cudaSuccess) return DM_ERR_ALLOC;
+            if (cudaMemcpyAsync(p->band_slots, slots.data(), slots.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, p->stream) !=
+                    cudaSuccess ||
+                cudaStreamSynchronize(p->stream) != cudaSuccess)
+                return DM_ERR_CUDA;
+            p->gd.band_slots = p->band_slots;
+            p->gd.n_band_slots = (int)slots.size();
+        }
+    }
+    return DM_OK;
 }
 
 int dm_plan_set_option(dm_plan* p, int option, double value)
@@ -729,6 +778,7 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->dc_total);
     cudaFree(p->dot_part);
     cudaFree(p->face_w);
+    cudaFree(p->band_slots);
     cudaFree(p->band_z);
     cudaFree(p->spec3);
     cudaFree(p->psfg_part);

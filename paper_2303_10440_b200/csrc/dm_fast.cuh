@@ -136,14 +136,23 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
     __shared__ float4 tile[(DM_FAST_TILE + 1) * 3];              // +1: halo record (edge of the step before the tile)
     __shared__ uint32_t flagw[(DM_FAST_TILE / 32) * DM_FAST_THREADS];
     const int tid = threadIdx.x;
-    // threads cover only the z-frequencies 0..nzb-1 that can be inside the narrow band (nzb = nzh without a band)
-    const long long n_thr = (long long)(ix_end - ix_begin) * n_yruns * grid.nzb;
+    // one thread per (i_x, y-run, i_z); under the narrow band only the listed threads (those with a frequency in the band)
+    const long long n_thr = grid.band_slots ? (long long)grid.n_band_slots : (long long)(ix_end - ix_begin) * n_yruns * grid.nzh;
     const long long lin = (long long)blockIdx.x * DM_FAST_THREADS + tid;
-    const bool in_range = lin < n_thr;
+    bool in_range = lin < n_thr;
     const long long l = in_range ? lin : 0;
-    const int iz = (int)(l % grid.nzb);
-    const int yrun = (int)((l / grid.nzb) % n_yruns);
-    const int ix = ix_begin + (int)(l / ((long long)grid.nzb * n_yruns));
+    int iz, yrun, ix;
+    if (grid.band_slots) {
+        const uint32_t s = grid.band_slots[l];
+        iz = (int)(s & 511u);
+        yrun = (int)((s >> 9) & 2047u);
+        ix = (int)(s >> 20);
+        in_range = in_range && ix >= ix_begin && ix < ix_end;
+    } else {
+        iz = (int)(l % grid.nzh);
+        yrun = (int)((l / grid.nzh) % n_yruns);
+        ix = ix_begin + (int)(l / ((long long)grid.nzh * n_yruns));
+    }
     const int nx = dm_signed_freq(ix, grid.nx), nz = iz;
     const int nys0 = -(grid.ny / 2) + yrun * DM_K;               // first signed y-frequency of the run
     const float hmax2 = __uint_as_float(*hmax2_bits);

@@ -20,6 +20,8 @@ struct DmGridDev {
     float band_cov[6];        // xx yy zz xy xz yz
     float band_lim;
     const float* face_w;      // per-face density weights, device [n_faces]; nullptr = all 1
+    const uint32_t* band_slots;  // narrow band: the forward kernel's active threads, packed i_x << 20 | y-run << 9 | i_z
+    int n_band_slots;            // (device, built by dm_plan_set_narrow_band); nullptr / 0 without a band
     int nzb;                  // stored z-frequencies 0..nzb-1 can be inside the band (nzb = nzh when the band is off)
 };
 
