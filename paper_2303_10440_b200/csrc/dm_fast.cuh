@@ -27,6 +27,9 @@
 static_assert(DM_STRIP_UNROLL == 6, "the strip loop is unrolled by 6 (window period 3 x gap ping-pong 2)");
 #define DM_K 8                      // frequencies per thread (run along y)
 #define DM_FAST_THREADS 128
+#ifndef DM_FAST_MINCTA
+#define DM_FAST_MINCTA 3            // resident CTAs per SM the register allocation aims at (160 registers: faster than 4 x 128)
+#endif
 #ifndef DM_FAST_TILE
 #define DM_FAST_TILE 384            // strip records per shared-memory tile (multiple of DM_STRIP_UNROLL and of 32)
 #endif
@@ -128,7 +131,7 @@ __device__ __forceinline__ float dm_gap_product(float dp, float dn, float& df)
 // grid = (k-blocks of DM_FAST_THREADS threads, n_chunks).  part[chunk][k] receives this chunk's partial sum, already
 // multiplied by the volume-mode prefactor i/|k|^2.
 template <int MODE>
-__global__ void __launch_bounds__(DM_FAST_THREADS, 4)
+__global__ void __launch_bounds__(DM_FAST_THREADS, DM_FAST_MINCTA)
 dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ chunk_off, DmGridDev grid, int ix_begin,
                   int ix_end, int n_yruns, float tau, const unsigned int* __restrict__ hmax2_bits, size_t part_stride,
                   float2* __restrict__ part)
