@@ -109,6 +109,9 @@ int backward_splits(const dm_plan* p, int* rows_per_split)
     int want = (p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
     if (p->band_on) want = std::max(want, std::min(p->n_split_max, 64));   // rows differ in cost under the narrow band:
                                                                              // many small CTAs balance the load
+    // a CTA sets up its seed table and records once: give it at least ~512 frequencies per triangle
+    const int min_rows = (512 + p->gd.nzh - 1) / p->gd.nzh;
+    if (want > n_rows / min_rows) want = n_rows / min_rows;
     if (want < 1) want = 1;
     if (want > n_rows) want = n_rows;
     if (want > p->n_split_max) want = p->n_split_max;
