@@ -281,7 +281,7 @@ def run_ours(args):
             "bound": "alu", "kernel": "dm_k_backward (A6, dominant)", "achieved": achieved, "peak": peak,
             "unit": "T lane-op/s (FP32 issue: 128 lanes/clk/SM)", "frac": achieved / peak, "traffic": None,
             "traffic_note": "ncu --set full needs an x-slab launch for valid counters: 12.2 MB DRAM per 1.36e10-pair launch "
-                            "(profiles/r01d_ncu_fast_kernels.txt); the kernel is compute-bound",
+                            "(profiles/r01e_ncu_fast_kernels.txt); the kernel is compute-bound",
             "peak_source": f"128 x {n_sm} SMs x {sm_max_mhz:.0f} MHz ({peak_src}); DESIGN.md section 7",
             "frac_at_measured_clock": achieved / (peak * sm_mhz / sm_max_mhz),
             "algorithmic_ops_per_pair": FLOOR_OPS["bwd"][w.mode], "kernel_ms": bk_ms,
