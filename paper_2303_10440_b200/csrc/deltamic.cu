@@ -247,11 +247,7 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     // seed spacing of the fast kernel: the smallest SEG whose seed table (ceil(nzh/SEG)-1 entries x 128 threads x 8 B,
     // one vertex slot per thread) has at most 8 entries per vertex
     const int nzh = p->gd.nzh;
-#if defined(DM_BF_FORCE_SEG)
-    const int seg = DM_BF_FORCE_SEG;
-#else
     const int seg = nzh <= 72 ? 8 : (nzh <= 144 ? 16 : 32);
-#endif
     const int n_seed = (nzh + seg - 1) / seg - 1;
     const size_t row_smem = 2 * (size_t)nzh * sizeof(float4) + (size_t)n_seed * DM_BF_THREADS * sizeof(float2) +
                             (size_t)(DM_BF_THREADS / 32) * DM_BF_STAGE * DM_PATCH_MAXV * sizeof(float2);
