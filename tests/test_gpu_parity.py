@@ -396,3 +396,24 @@ def test_per_face_density_weights(dm, mode):
     F1 = plan.mesh_ft_forward(_dev(v)).cpu().numpy().reshape(-1)
     assert np.abs(F1 - oracle.mesh_ft_forward(v, f, k, mode)).max() <= FWD_TOL * abs(ref[0])
     plan.close()
+
+
+def test_sharded_backward_helper_single_rank_and_emulated_ranks(dm):
+    """paper_2303_10440_b200.sharding on the GPU: without a process group the helper is the whole-grid backward; the
+    partial gradients of the slabs of three emulated ranks (run one after the other, as the profiling guide asks for
+    multi-rank paths on one GPU) add up to it."""
+    import torch
+    from paper_2303_10440_b200.sharding import sharded_mesh_ft_backward, slab_bounds
+    w = build_workload(2, subdiv_override=2, grid_override=(20, 16, 16))
+    plan, vd = _plan(dm, w), _dev(w.vertices)
+    Gd = _dev(spectrum_cotangent(w))
+    whole = plan.mesh_ft_backward(vd, Gd).clone()
+    assert torch.equal(sharded_mesh_ft_backward(plan, vd, Gd), whole)
+    total = torch.zeros_like(whole)
+    for rank in range(3):
+        b, e = slab_bounds(w.n[0], 3, rank)
+        plan.set_slab(b, e)
+        total += plan.mesh_ft_backward(vd, Gd)
+    plan.set_slab(0, w.n[0])
+    assert float(torch.linalg.norm(total - whole) / torch.linalg.norm(whole)) <= 1e-5
+    plan.close()
