@@ -201,12 +201,12 @@ int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
                                                                       n_yruns, p->tau, p->hmax2, stride, p->fwd_part);
     if ((rc = check_launch(p))) return rc;
     const int W = 2 * DM_LOWK_BOX + 1;
-    const unsigned lowk_blocks = (unsigned)((W * W * (DM_LOWK_BOX + 1) + 3) / 4);
+    const unsigned lowk_blocks = (unsigned)(W * W * (DM_LOWK_BOX + 1));   // one CTA per frequency of the low-k box
     if (p->mode == DM_SURFACE)
-        dm_k_forward_lowk<1><<<lowk_blocks, 128, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
+        dm_k_forward_lowk<1><<<lowk_blocks, DM_LOWK_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
                                                                  p->ix_end, p->hmax2, (float2*)F_dev);
     else
-        dm_k_forward_lowk<0><<<lowk_blocks, 128, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
+        dm_k_forward_lowk<0><<<lowk_blocks, DM_LOWK_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
                                                                  p->ix_end, p->hmax2, (float2*)F_dev);
     if ((rc = check_launch(p))) return rc;
     const long long n_slab = (long long)(p->ix_end - p->ix_begin) * p->gd.ny * p->gd.nzh;

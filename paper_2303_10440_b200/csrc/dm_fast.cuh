@@ -295,17 +295,20 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
     }
 }
 
-// ---- A4 at low |k|: every pair through the robust branches; one WARP per frequency, lanes stride over the records ----
-// Thread block = 4 warps = 4 frequencies of the low-k box; writes F directly.
+// ---- A4 at low |k|: every pair through the robust branches; one CTA per frequency, threads stride over the records ----
+// grid = the (2B+1)^2 (B+1) frequencies of the low-k box (most CTAs leave at once); writes F directly.  The block sum is
+// taken in a fixed order (lane tree, then the warps in order): deterministic.
+#define DM_LOWK_THREADS 256
 template <int MODE>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(DM_LOWK_THREADS)
 dm_k_forward_lowk(const float4* __restrict__ rec, const int32_t* __restrict__ chunk_off, int n_chunks, DmGridDev grid,
                   int ix_begin, int ix_end, const unsigned int* __restrict__ hmax2_bits, float2* __restrict__ F)
 {
+    __shared__ float wsum[2][DM_LOWK_THREADS / 32];
     const int B = DM_LOWK_BOX, W = 2 * B + 1;
-    const int warp = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (warp >= W * W * (B + 1)) return;
-    const int nz = warp % (B + 1), nys = (warp / (B + 1)) % W - B, nx = warp / ((B + 1) * W) - B;
+    const int fi = blockIdx.x, lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+    if (fi >= W * W * (B + 1)) return;
+    const int nz = fi % (B + 1), nys = (fi / (B + 1)) % W - B, nx = fi / ((B + 1) * W) - B;
     if (nz > grid.nz / 2 || nys < -(grid.ny / 2) || nys > (grid.ny - 1) / 2 || nx < -(grid.nx / 2) || nx > (grid.nx - 1) / 2) return;
     const int ix = nx < 0 ? nx + grid.nx : nx, iy = nys < 0 ? nys + grid.ny : nys;
     if (ix < ix_begin || ix >= ix_end) return;
@@ -314,7 +317,7 @@ dm_k_forward_lowk(const float4* __restrict__ rec, const int32_t* __restrict__ ch
     float are = 0.f, aim = 0.f;
     for (int c = 0; c < n_chunks; ++c) {
         const int b = chunk_off[c], e = chunk_off[c + 1];
-        for (int i = b + 1 + lane; i < e; i += 32) {   // record b closes no triangle
+        for (int i = b + 1 + (int)threadIdx.x; i < e; i += DM_LOWK_THREADS) {   // record b closes no triangle
             const float4 r2 = rec[3 * (size_t)i + 2];
             const bool valid = (MODE == 1) ? (r2.x != 0.f) : (r2.x != 0.f || r2.y != 0.f || r2.z != 0.f);
             if (!valid) continue;
@@ -336,6 +339,17 @@ dm_k_forward_lowk(const float4* __restrict__ rec, const int32_t* __restrict__ ch
         aim += __shfl_xor_sync(0xffffffffu, aim, o);
     }
     if (lane == 0) {
+        wsum[0][wrp] = are;
+        wsum[1][wrp] = aim;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        are = 0.f, aim = 0.f;
+#pragma unroll
+        for (int w = 0; w < DM_LOWK_THREADS / 32; ++w) {
+            are += wsum[0][w];
+            aim += wsum[1][w];
+        }
         if (MODE == 0) {
             const float k2 = kx * kx + ky * ky + kz * kz;
             const float ik2 = (k2 > 0.f) ? 1.0f / k2 : 0.f;
