@@ -46,7 +46,7 @@ struct dm_plan {
     int st_n_rec = 0, st_n_chunks = 0;
     float4* st_rec = nullptr;        // [st_n_rec*3] strip records (A1)
     float2* fwd_part = nullptr;      // [st_n_chunks * n_k] per-chunk partial spectra
-    unsigned int* hmax2 = nullptr;   // longest squared edge (float bits), rebuilt every call
+    unsigned int* hmax2 = nullptr;   // 16 bytes of edge statistics (dm_edge_stats_add), rebuilt every call
     double* dc_part = nullptr;       // [DM_DC_BLOCKS] block sums of the k = 0 entry
     bool normalise = false;          // DM_OPT_AREA_NORMALISED (surface mode): u = F/|Lambda|, eq. 12-13
     double* dc_total = nullptr;      // [1] fp64 volume / total area of the last forward (k = 0 kernels)
@@ -182,7 +182,7 @@ int run_forward_robust(dm_plan* p, const float* vertices_dev, float* F_dev)
 
 int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
 {
-    if (cudaMemsetAsync(p->hmax2, 0, sizeof(unsigned int), p->stream) != cudaSuccess) return DM_ERR_CUDA;
+    if (cudaMemsetAsync(p->hmax2, 0, 16, p->stream) != cudaSuccess) return DM_ERR_CUDA;
     DmStripDev st = {p->st_new, p->st_prev, p->st_ret, p->st_fid, p->st_n_rec};
     dm_k_strip_geometry<<<(p->st_n_rec + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, st, p->gd, p->mode,
                                                                            p->st_rec, p->hmax2);
@@ -255,7 +255,9 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     if (p->bwd_path == 0 && nzh <= 288) {
         const DmPatchDev pt = {p->pt_face, p->pt_vid, p->pt_loc, p->pt_lanes};
         grid.x = (unsigned)(p->pt_lanes / DM_BF_THREADS);
-        dm_k_bwd_geometry<<<(p->pt_lanes + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, pt, p->gd, p->btrec, p->bvrec);
+        if (cudaMemsetAsync(p->hmax2, 0, 16, p->stream) != cudaSuccess) return DM_ERR_CUDA;
+        dm_k_bwd_geometry<<<(p->pt_lanes + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, pt, p->gd, p->btrec, p->bvrec,
+                                                                                  p->hmax2);
         if ((rc = check_launch(p))) return rc;
 #define DM_LAUNCH_BF2(MODE, SEG, BAND)                                                                                   \
     do {                                                                                                                 \
@@ -264,7 +266,7 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
             return DM_ERR_CUDA;                                                                                          \
         dm_k_backward_fast<MODE, SEG, BAND><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(                               \
             p->btrec, p->bvrec, pt, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, p->tau_b, (const float2*)G_dev,      \
-            p->band_z, p->part);                                                                                         \
+            p->band_z, p->part);                                                                                                 \
     } while (0)
 #define DM_LAUNCH_BF(MODE, SEG)                                                                                          \
     do {                                                                                                                 \
@@ -394,6 +396,12 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
     p->gd.band_slots = nullptr;
     p->gd.n_band_slots = 0;
     p->gd.face_w = nullptr;
+    {
+        double lmax = 0.0;
+        for (int dd = 0; dd < 3; ++dd) lmax = std::max(lmax, (double)grid->n[dd] * (double)grid->spacing[dd]);
+        p->gd.edge_fix = (float)(1073741824.0 / (lmax * lmax));   // squared edges in units of 2^-30 L_max^2
+        p->gd.inv_edge_norm = (float)(1.0 / (3.0 * (double)n_faces * (double)p->gd.edge_fix));
+    }
     p->ix_begin = 0;
     p->ix_end = p->gd.nx;
     // gap-product threshold of the forward fast path: one excluded-or-not pair may cost ~1e-6 (sum|d|)/tau of ONE
@@ -464,7 +472,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
                 cudaMalloc(&p->st_chunk_off, sr.chunk_off.size() * sizeof(int32_t)) != cudaSuccess ||
                 cudaMalloc(&p->st_rec, (size_t)p->st_n_rec * 3 * sizeof(float4)) != cudaSuccess ||
                 cudaMalloc(&p->fwd_part, (size_t)p->st_n_chunks * nk * sizeof(float2)) != cudaSuccess ||
-                cudaMalloc(&p->hmax2, sizeof(unsigned int)) != cudaSuccess ||
+                cudaMalloc(&p->hmax2, 16) != cudaSuccess ||
                 cudaMalloc(&p->dc_part, DM_DC_BLOCKS * sizeof(double)) != cudaSuccess ||
                 cudaMalloc(&p->dc_total, sizeof(double)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
             if (cudaMemcpyAsync(p->st_new, sr.vid_new.data(), nb, cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||

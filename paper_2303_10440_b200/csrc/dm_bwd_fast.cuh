@@ -64,13 +64,15 @@ struct DmPatchDev {
 
 // Records rebuilt every call (row A1), indexed by lane i = 32 * patch + l:
 //   triangle  trec[4i..4i+3] = (u_0.xyz [uint32 bit patterns: v_0 / L in fixed-point turns], loc bits)
-//                              (eb.xyz, -)   (ec.xyz, -)   (m_T.xyz, |m_T|)       eb = v_1-v_0, ec = v_2-v_0
+//                              (eb.xyz, longest squared edge)   (ec.xyz, -)   (m_T.xyz, |m_T|)       eb = v_1-v_0, ec = v_2-v_0
 //   vertex    vrec[2i..2i+1] (slot l of the patch):  (u.xyz turns, rho.re)  (rho.im, -, -, -),  rho = e^{-i kstep_z v_z}
 __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int32_t* __restrict__ faces, DmPatchDev pt,
-                                  DmGridDev grid, float4* __restrict__ trec, float4* __restrict__ vrec)
+                                  DmGridDev grid, float4* __restrict__ trec, float4* __restrict__ vrec,
+                                  unsigned int* __restrict__ hmax2_bits)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= pt.n_lanes) return;
+    if (i >= pt.n_lanes) return;   // n_lanes is a multiple of the warp size: whole warps leave
+    float h2 = 0.f, e2sum = 0.f;
     {
         int f = pt.face[i];
         if (f < 0) f = pt.face[i & ~31];   // idle lane: any valid triangle of the patch (lane 0 holds one)
@@ -93,12 +95,20 @@ __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int3
         const float ec[3] = {v[2][0] - v[0][0], v[2][1] - v[0][1], v[2][2] - v[0][2]};
         float m[3];
         dm_cross(eb, ec, m);
+        // edge statistics of the mesh (they scale the flag threshold)
+        const float ed[3] = {ec[0] - eb[0], ec[1] - eb[1], ec[2] - eb[2]};
+        const float a2 = eb[0] * eb[0] + eb[1] * eb[1] + eb[2] * eb[2], b2 = ec[0] * ec[0] + ec[1] * ec[1] + ec[2] * ec[2],
+                    c2 = ed[0] * ed[0] + ed[1] * ed[1] + ed[2] * ed[2];
+        if (pt.face[i] >= 0) {
+            h2 = fmaxf(fmaxf(a2, b2), c2);
+            e2sum = a2 + b2 + c2;
+        }
         const float wf = grid.face_w ? grid.face_w[f] : 1.0f;   // density weight of the face
         const float mn = wf * sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
         m[0] *= wf, m[1] *= wf, m[2] *= wf;
         float4* o = trec + (size_t)DM_BF_TREC * i;
         o[0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), __uint_as_float(pt.loc[i]));
-        o[1] = make_float4(eb[0], eb[1], eb[2], 0.f);
+        o[1] = make_float4(eb[0], eb[1], eb[2], fmaxf(fmaxf(a2, b2), c2));
         o[2] = make_float4(ec[0], ec[1], ec[2], 0.f);
         o[3] = make_float4(m[0], m[1], m[2], mn);
     }
@@ -124,6 +134,7 @@ __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int3
         vrec[DM_BF_VREC * s] = a;
         vrec[DM_BF_VREC * s + 1] = b;
     }
+    dm_edge_stats_add(hmax2_bits, h2, e2sum, grid.edge_fix);
 }
 
 // shared-memory queue of one warp's flagged pairs of one chunk
@@ -160,15 +171,16 @@ __device__ __forceinline__ void dm_bf_add(DmBfRow& a, float kz, float om, float 
 template <int MODE>
 __device__ __forceinline__ bool dm_bf_pair(const float kz, const cf A0, const cf A1, const cf A2, const float prow,
                                            const float qrow, const float omrow, const float ebz, const float ecz,
-                                           const float mz, const float tau_b, DmBfRow& rs)
+                                           const float mz, const float tau_k, DmBfRow& rs)
 {
     const float p = fmaf(kz, ebz, prow), q = fmaf(kz, ecz, qrow), r = q - p;
     const float pqr = (p * q) * r;
     // the largest derivative coefficient is 1/(m1^2 m2), m1 <= m2 <= m3 the sorted |gaps| (m3 = m1 + m2 always): the pair
-    // leaves the fast path when m1^2 m2 = m1 |pqr| / m3 <= tau_b  (also catches p = q = r = 0)
+    // leaves the fast path when m1^2 m2 = m1 |pqr| / m3 <= tau_k  (also catches p = q = r = 0); tau_k = the threshold of
+    // this triangle on this row (tau_b, larger for a triangle that is coarse for the grid)
     const float m1 = fminf(fminf(fabsf(p), fabsf(q)), fabsf(r));
     const float m3 = fmaxf(fmaxf(fabsf(p), fabsf(q)), fabsf(r));
-    const bool bad = !(m1 * fabsf(pqr) > tau_b * m3);
+    const bool bad = !(m1 * fabsf(pqr) > tau_k * m3);
     const float R = bad ? 0.f : dm_rcp_approx(pqr);
     const float c0 = -r * R, c1 = q * R, c2 = -p * R;
     const float c0s = c0 * c0, c1s = c1 * c1, c2s = c2 * c2;
@@ -274,7 +286,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
     // one stage of n <= DM_BF_STAGE frequencies starting at z: every lane writes A_v of its vertex slot(s), then every
     // lane evaluates its triangle at those frequencies; returns the flags of the stage (bit j = frequency z + j)
     auto run_stage = [&](const float4* skr, int z, int n, bool full, cf& Ea, float prow, float qrow, float omrow,
-                         DmBfRow& rs) -> uint32_t {
+                         float tau_row, DmBfRow& rs) -> uint32_t {
         if (full) {
 #pragma unroll
             for (int j = 0; j < DM_BF_STAGE; ++j) {
@@ -300,7 +312,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
                 const float kz = skr[z + j].z;
                 const float2 a0 = at[j * DM_PATCH_MAXV + l0], a1 = at[j * DM_PATCH_MAXV + l1], a2 = at[j * DM_PATCH_MAXV + l2];
                 if (dm_bf_pair<MODE>(kz, cf{a0.x, a0.y}, cf{a1.x, a1.y}, cf{a2.x, a2.y}, prow, qrow, omrow, r3.z, r4.z, r5.z,
-                                     tau_b, rs))
+                                     tau_row, rs))
                     sf |= 1u << j;
             }
         } else {
@@ -309,7 +321,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
                 const float kz = skr[z + j].z;
                 const float2 a0 = at[j * DM_PATCH_MAXV + l0], a1 = at[j * DM_PATCH_MAXV + l1], a2 = at[j * DM_PATCH_MAXV + l2];
                 if (dm_bf_pair<MODE>(kz, cf{a0.x, a0.y}, cf{a1.x, a1.y}, cf{a2.x, a2.y}, prow, qrow, omrow, r3.z, r4.z, r5.z,
-                                     tau_b, rs))
+                                     tau_row, rs))
                     sf |= 1u << j;
             }
         }
@@ -328,6 +340,12 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
         const float prow = fmaf(kx, r3.x, ky * r3.y), qrow = fmaf(kx, r4.x, ky * r4.y);
         const float omrow = fmaf(kx, r5.x, ky * r5.y);
+        // flag threshold of this triangle on this row: tau_b max(1, (|k| h_T / 12)^3), |k| the largest of the row, h_T the
+        // longest edge of the triangle.  On a triangle that is large for the grid (|k| h >> 1) the rounding error of a gap
+        // k.e grows like |k| h while the integral decays like 1/(|k| h)^2; the factor is exactly 1 when |k| h_T <= 12
+        const float kzm = grid.kstep[2] * (float)(nzh - 1);
+        const float kh2 = (1.0f / 144.0f) * (kx * kx + ky * ky + kzm * kzm) * r3.w;
+        const float tau_row = tau_b * fmaxf(1.0f, kh2 * sqrtf(kh2));
         // exact row phase e^{-i (k_x v_x + k_y v_y)} of the lane's vertex slot
         const cf Xa = dm_expmi_turns((uint32_t)nx * uax + (uint32_t)ny * uay);
         DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -367,12 +385,12 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
                         if (len == DM_BF_UNR) {
 #pragma unroll
                             for (int h = 0; h < DM_BF_UNR / DM_BF_STAGE; ++h)
-                                sf |= run_stage(skr, z0 + h * DM_BF_STAGE, DM_BF_STAGE, true, Ea, prow, qrow, omrow, rs)
+                                sf |= run_stage(skr, z0 + h * DM_BF_STAGE, DM_BF_STAGE, true, Ea, prow, qrow, omrow, tau_row, rs)
                                       << (h * DM_BF_STAGE);
                         } else {
 #pragma unroll 1
                             for (int j0 = 0; j0 < len; j0 += DM_BF_STAGE)
-                                sf |= run_stage(skr, z0 + j0, min(DM_BF_STAGE, len - j0), false, Ea, prow, qrow, omrow, rs) << j0;
+                                sf |= run_stage(skr, z0 + j0, min(DM_BF_STAGE, len - j0), false, Ea, prow, qrow, omrow, tau_row, rs) << j0;
                         }
                         word |= sf << (s * DM_BF_UNR);
                     }

@@ -53,7 +53,7 @@ __global__ void dm_k_strip_geometry(const float* __restrict__ vertices, const in
                                     DmGridDev grid, int mode, float4* __restrict__ rec, unsigned int* __restrict__ hmax2_bits)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    float h2 = 0.f;
+    float h2 = 0.f, e2sum = 0.f;
     if (i < st.n_rec) {
         const int vn = st.vid_new[i], vp = st.vid_prev[i], vr = max(st.vid_ret[i], 0), f = st.fid[i];
         uint32_t u[3];
@@ -87,18 +87,18 @@ __global__ void dm_k_strip_geometry(const float* __restrict__ vertices, const in
             const float wf = grid.face_w ? grid.face_w[f] : 1.0f;   // density weight of the face
             if (mode == 1) r2.x = wf * sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
             else r2 = make_float4(wf * m[0], wf * m[1], wf * m[2], 0.f);
-            // longest edge of the triangle (squared)
+            // longest edge of the triangle (squared) and the sum of its squared edges
             const float c[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]};
-            h2 = fmaxf(fmaxf(a[0] * a[0] + a[1] * a[1] + a[2] * a[2], b[0] * b[0] + b[1] * b[1] + b[2] * b[2]),
-                       c[0] * c[0] + c[1] * c[1] + c[2] * c[2]);
+            const float a2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2], b2 = b[0] * b[0] + b[1] * b[1] + b[2] * b[2],
+                        c2 = c[0] * c[0] + c[1] * c[1] + c[2] * c[2];
+            h2 = fmaxf(fmaxf(a2, b2), c2);
+            e2sum = a2 + b2 + c2;
         }
         rec[3 * (size_t)i + 0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), (float)cs);
         rec[3 * (size_t)i + 1] = make_float4((float)(-sn), e[0], e[1], e[2]);
         rec[3 * (size_t)i + 2] = r2;
     }
-    // block max of the squared edge length -> one atomicMax per block (non-negative floats order like their bit patterns)
-    for (int o = 16; o > 0; o >>= 1) h2 = fmaxf(h2, __shfl_xor_sync(0xffffffffu, h2, o));
-    if ((threadIdx.x & 31) == 0 && h2 > 0.f) atomicMax(hmax2_bits, __float_as_uint(h2));
+    dm_edge_stats_add(hmax2_bits, h2, e2sum, grid.edge_fix);
 }
 
 // "low" frequencies: |k| h_max < DM_LOWK_RADIUS (every triangle has only small gaps there) and inside the box the
@@ -158,15 +158,22 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
     }
     const int nx = dm_signed_freq(ix, grid.nx), nz = iz;
     const int nys0 = -(grid.ny / 2) + yrun * DM_K;               // first signed y-frequency of the run
-    const float hmax2 = __uint_as_float(*hmax2_bits);
+    const float hmax2 = __uint_as_float(*hmax2_bits), hmean2 = dm_edge_mean2(hmax2_bits, grid);
     const float kx = grid.kstep[0] * nx, kz = grid.kstep[2] * nz;
     float kyj[DM_K], tauj[DM_K];    // tauj < 0 switches a low frequency off (never flagged; its sums are not stored)
+    // On a mesh that is coarse for the grid (|k| h >> 1) the rounding error of a gap k.e grows like |k| h while the
+    // triangle integral itself decays like 1/(|k| h)^2, so the threshold scales with max(1, (|k| h_rms / 10)^3): exactly 1 on
+    // meshes whose edges are a few voxels long (the benchmark configurations), larger on coarse meshes.
+    // One value per thread, taken at the largest |k| of its run.
+    const float kye = fmaxf(fabsf(grid.kstep[1] * (float)nys0), fabsf(grid.kstep[1] * (float)(nys0 + DM_K - 1)));
+    const float kh2 = 0.01f * (kx * kx + kye * kye + kz * kz) * hmean2;   // (|k| h_rms / 10)^2
+    const float tau_t = tau * fmaxf(1.0f, kh2 * sqrtf(kh2));
     bool live = false;
 #pragma unroll
     for (int j = 0; j < DM_K; ++j) {
         kyj[j] = __fmul_rn(grid.kstep[1], (float)(nys0 + j));
         const bool low = dm_k_is_low(grid, nx, nys0 + j, nz, hmax2) || !dm_in_band(grid, nx, nys0 + j, nz);
-        tauj[j] = low ? -1.0f : tau;
+        tauj[j] = low ? -1.0f : tau_t;
         live |= !low;
     }
     live &= in_range;

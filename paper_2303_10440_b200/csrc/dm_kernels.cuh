@@ -19,11 +19,35 @@ struct DmGridDev {
     // the Gaussian PSF of covariance B, band_lim = ln(1/cutoff)); band_lim = +inf switches the band off
     float band_cov[6];        // xx yy zz xy xz yz
     float band_lim;
+    float edge_fix;           // fixed-point scale of the squared edge lengths summed by the geometry kernels
+    float inv_edge_norm;      // 1 / (3 n_faces edge_fix): mean squared edge = sum * inv_edge_norm
     const float* face_w;      // per-face density weights, device [n_faces]; nullptr = all 1
     const uint32_t* band_slots;  // narrow band: the forward kernel's active threads, packed i_x << 20 | y-run << 9 | i_z
     int n_band_slots;            // (device, built by dm_plan_set_narrow_band); nullptr / 0 without a band
     int nzb;                  // stored z-frequencies 0..nzb-1 can be inside the band (nzb = nzh when the band is off)
 };
+
+// Edge statistics of the mesh, rebuilt by the geometry kernel of every call in a 16-byte device buffer:
+//   word 0 = longest squared edge (float bits; non-negative floats order like their bit patterns), bytes 8..15 = sum of
+//   the squared edges of all faces in fixed point (integer adds: the sum does not depend on the order of the atomics).
+// dm_edge_stats_add is called by every thread of a warp (val = 0, h2 = 0 for threads without a face).
+__device__ __forceinline__ void dm_edge_stats_add(unsigned int* stats, float h2max, float e2sum, float edge_fix)
+{
+    unsigned long long s = (unsigned long long)(e2sum * edge_fix);
+    for (int o = 16; o > 0; o >>= 1) {
+        h2max = fmaxf(h2max, __shfl_xor_sync(0xffffffffu, h2max, o));
+        s += __shfl_xor_sync(0xffffffffu, s, o);
+    }
+    if ((threadIdx.x & 31) == 0 && h2max > 0.f) {
+        atomicMax(stats, __float_as_uint(h2max));
+        atomicAdd(reinterpret_cast<unsigned long long*>(stats) + 1, s);
+    }
+}
+// mean squared edge length of the mesh
+__device__ __forceinline__ float dm_edge_mean2(const unsigned int* stats, const DmGridDev& grid)
+{
+    return (float)(reinterpret_cast<const unsigned long long*>(stats)[1]) * grid.inv_edge_norm;
+}
 
 __device__ __forceinline__ bool dm_in_band(const DmGridDev& grid, int nx, int ny, int nz)
 {

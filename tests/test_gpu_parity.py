@@ -417,3 +417,30 @@ def test_sharded_backward_helper_single_rank_and_emulated_ranks(dm):
     plan.set_slab(0, w.n[0])
     assert float(torch.linalg.norm(total - whole) / torch.linalg.norm(whole)) <= 1e-5
     plan.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_coarse_meshes_large_gaps(dm, mode):
+    """Meshes that are coarse for the grid (|k| h up to ~90, the regime of the paper's 80-triangle sphere of Fig. 6,
+    PAPER.md:221): a 20-triangle and an 80-triangle sphere, and a fine sphere next to a coarse one.  The flag thresholds
+    scale with (|k| h)^3 there; forward and gradient must stay within the tolerances."""
+    import torch
+    rng = np.random.default_rng(35)
+    meshes = []
+    for sub, R in ((0, 0.4), (1, 0.3)):
+        v, f = icosphere(sub, R, (0.03, -0.02, 0.05))
+        meshes.append((v.astype(np.float32), f))
+    va, fa = icosphere(0, 0.17, (-0.25, 0.1, 0.05))
+    vb, fb = icosphere(2, 0.15, (0.2, -0.1, 0.0))
+    meshes.append((np.vstack([va, vb]).astype(np.float32), np.vstack([fa, fb + len(va)]).astype(np.int32)))
+    n, spacing = (38, 22, 24), (1.35 / 38, 1.53 / 22, 0.77 / 24)
+    for v, f in meshes:
+        plan = dm.Plan(n, spacing, (-0.6, -0.7, -0.35), mode, torch.as_tensor(f, device="cuda"), v.shape[0])
+        F = plan.mesh_ft_forward(_dev(v)).cpu().numpy()
+        ref = oracle.mesh_ft_forward_grid(v, f, n, spacing, mode)
+        assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0])
+        G = (rng.standard_normal(ref.shape) + 1j * rng.standard_normal(ref.shape)).astype(np.complex64)
+        dv = plan.mesh_ft_backward(_dev(v), _dev(G)).cpu().numpy()
+        dref = oracle.mesh_ft_backward_grid(v, f, n, spacing, mode, G.astype(np.complex128))
+        assert _rel_l2(dv, dref) <= GRAD_TOL, (len(f), _rel_l2(dv, dref))
+        plan.close()
