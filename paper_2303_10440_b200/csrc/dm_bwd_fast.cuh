@@ -344,7 +344,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         // longest edge of the triangle.  On a triangle that is large for the grid (|k| h >> 1) the rounding error of a gap
         // k.e grows like |k| h while the integral decays like 1/(|k| h)^2; the factor is exactly 1 when |k| h_T <= 12
         const float kzm = grid.kstep[2] * (float)(nzh - 1);
-        const float kh2 = (1.0f / 144.0f) * (kx * kx + ky * ky + kzm * kzm) * r3.w;
+        const float kh2 = (1.0f / 144.0f) * (kx * kx + ky * ky + kzm * kzm) * trec[tid * DM_BF_TREC + 1].w;   // (re-read: one register less)
         const float tau_row = tau_b * fmaxf(1.0f, kh2 * sqrtf(kh2));
         // exact row phase e^{-i (k_x v_x + k_y v_y)} of the lane's vertex slot
         const cf Xa = dm_expmi_turns((uint32_t)nx * uax + (uint32_t)ny * uay);
