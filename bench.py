@@ -281,11 +281,11 @@ def run_ours(args):
             "bound": "alu", "kernel": "dm_k_backward (A6, dominant)", "achieved": achieved, "peak": peak,
             "unit": "T lane-op/s (FP32 issue: 128 lanes/clk/SM)", "frac": achieved / peak, "traffic": None,
             "traffic_note": "ncu --set full needs an x-slab launch for valid counters: 12.2 MB DRAM per 1.36e10-pair launch "
-                            "(profiles/r01e_ncu_fast_kernels.txt); the kernel is compute-bound",
+                            "(profiles/r01f_ncu_fast_kernels.txt); the kernel is compute-bound",
             "peak_source": f"128 x {n_sm} SMs x {sm_max_mhz:.0f} MHz ({peak_src}); DESIGN.md section 7",
             "frac_at_measured_clock": achieved / (peak * sm_mhz / sm_max_mhz),
             "algorithmic_ops_per_pair": FLOOR_OPS["bwd"][w.mode], "kernel_ms": bk_ms,
-            "ncu": {"issued_instr_per_pair": 86.9, "issue_active_pct": 80.6, "source": "profiles/r01e_ncu_fast_kernels.txt "
+            "ncu": {"issued_instr_per_pair": 87.3, "issue_active_pct": 79.8, "source": "profiles/r01f_ncu_fast_kernels.txt "
                     "(cfg 4 x-slab capture; static numbers, not measured by this run)"},
             "forward": {"achieved": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12,
                         "frac": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12 / peak,
