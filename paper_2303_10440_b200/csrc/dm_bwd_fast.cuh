@@ -49,7 +49,7 @@
 #define DM_BF_SEG 32            // bits of one flag word
 #define DM_BF_UNR 8             // unroll of the fast loop
 #ifndef DM_BF_STAGE
-#define DM_BF_STAGE 4           // frequencies whose vertex phases are staged in shared memory at a time (divides DM_BF_UNR)
+#define DM_BF_STAGE 8           // frequencies whose vertex phases are staged in shared memory at a time (divides DM_BF_UNR)
 #endif
 #define DM_BF_TREC 4            // float4 per triangle record
 #define DM_BF_VREC 2            // float4 per vertex-slot record
