@@ -285,7 +285,7 @@ def run_ours(args):
             "peak_source": f"128 x {n_sm} SMs x {sm_max_mhz:.0f} MHz ({peak_src}); DESIGN.md section 7",
             "frac_at_measured_clock": achieved / (peak * sm_mhz / sm_max_mhz),
             "algorithmic_ops_per_pair": FLOOR_OPS["bwd"][w.mode], "kernel_ms": bk_ms,
-            "ncu": {"issued_instr_per_pair": 87.3, "issue_active_pct": 79.8, "source": "profiles/r01f_ncu_fast_kernels.txt "
+            "ncu": {"issued_instr_per_pair": 85.8, "issue_active_pct": 79.5, "source": "profiles/r01f_ncu_fast_kernels.txt "
                     "(cfg 4 x-slab capture; static numbers, not measured by this run)"},
             "forward": {"achieved": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12,
                         "frac": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12 / peak,
