@@ -52,6 +52,7 @@ struct dm_plan {
     double* dc_total = nullptr;      // [1] fp64 volume / total area of the last forward (k = 0 kernels)
     double* dot_part = nullptr;      // [DM_DOT_BLOCKS + 1] block sums and result of sum_k Re(conj(G) F)
     float* face_w = nullptr;         // [n_faces] per-face density weights, valid while gd.face_w points at it
+    long long band_count = 0;        // stored frequencies inside the narrow band (whole grid)
     uint32_t* band_slots = nullptr;  // the forward kernel's thread list under the narrow band
     int2* band_z = nullptr;          // [nx*ny] in-band z interval of every row (narrow band), valid while band_on
     bool band_on = false;
@@ -247,6 +248,13 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     // seed spacing of the fast kernel: the smallest SEG whose seed table (ceil(nzh/SEG)-1 entries x 128 threads x 8 B,
     // one vertex slot per thread) has at most 8 entries per vertex
     const int nzh = p->gd.nzh;
+    // The flag threshold is calibrated for sums over many frequencies (errors of single pairs average out); when a vertex
+    // gradient sums fewer than ~5e4 frequencies (tiny grids, narrow bands, thin slabs) one pair just above the threshold
+    // could dominate, so the threshold grows like 1/sqrt(number of frequencies)
+    // (counted over the whole grid, not the slab: the slabs' partial gradients are summed afterwards)
+    double n_freq = (double)p->gd.nx * p->gd.ny * nzh;
+    if (p->band_on) n_freq = std::max(1.0, (double)p->band_count);
+    const float tau_b_eff = (float)((double)p->tau_b * std::max(1.0, std::sqrt(5.0e4 / n_freq)));
     const int seg = nzh <= 72 ? 8 : (nzh <= 144 ? 16 : 32);
     const int n_seed = (nzh + seg - 1) / seg - 1;
     const size_t row_smem = 2 * (size_t)nzh * sizeof(float4) + (size_t)n_seed * DM_BF_THREADS * sizeof(float2) +
@@ -265,7 +273,7 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
                                  (int)row_smem) != cudaSuccess)                                                          \
             return DM_ERR_CUDA;                                                                                          \
         dm_k_backward_fast<MODE, SEG, BAND><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(                               \
-            p->btrec, p->bvrec, pt, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, p->tau_b, (const float2*)G_dev,      \
+            p->btrec, p->bvrec, pt, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, tau_b_eff, (const float2*)G_dev,      \
             p->band_z, p->part);                                                                                                 \
     } while (0)
 #define DM_LAUNCH_BF(MODE, SEG)                                                                                          \
@@ -590,6 +598,8 @@ int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
     if (cudaMemcpyAsync(bz.data(), p->band_z, (size_t)n_rows * sizeof(int2), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
         cudaStreamSynchronize(p->stream) != cudaSuccess)
         return DM_ERR_CUDA;
+    p->band_count = 0;
+    for (const int2& b : bz) p->band_count += std::max(0, b.y - b.x);
     const int ny = p->gd.ny, n_yruns = (ny + DM_K - 1) / DM_K;
     if (p->gd.nx <= 4096 && n_yruns <= 2048 && p->gd.nzh <= 512) {
         try {
