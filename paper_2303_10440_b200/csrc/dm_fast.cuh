@@ -33,13 +33,15 @@ static_assert(DM_STRIP_UNROLL == 6, "the strip loop is unrolled by 6 (window per
 #ifndef DM_FAST_TILE
 #define DM_FAST_TILE 384            // strip records per shared-memory tile (multiple of DM_STRIP_UNROLL and of 32)
 #endif
+#define DM_FORCE_KH2 361.0f          // (|k| h_T)^2 above which a face skips the fast path of the forward kernel
 #define DM_LOWK_RADIUS 0.5f         // |k| h_max below which a frequency is "low" (all gaps small for all triangles)
 #define DM_LOWK_BOX 24              // low-k kernel covers |n_a| <= DM_LOWK_BOX
 
 // strip record = 3 x float4 (48 B):
 //   r0 = (u_ret.xyz [uint32 bit patterns], rho_ret.re)     retiring vertex: fixed-point position, y-rotation
 //   r1 = (rho_ret.im, e.xyz)                               e = v_new - v_prev
-//   r2 = surface: (|m_T|, 0, 0, 0)   volume: (m_T.xyz, 0)  zero when the step closes no triangle
+//   r2 = surface: (|m_T|, 0, 0, h2)   volume: (m_T.xyz, h2)  x..z zero when the step closes no triangle; h2 = longest
+//        squared edge of the face
 struct DmStripDev {
     const int32_t* vid_new;
     const int32_t* vid_prev;
@@ -85,7 +87,7 @@ __global__ void dm_k_strip_geometry(const float* __restrict__ vertices, const in
             float m[3];
             dm_cross(a, b, m);
             const float wf = grid.face_w ? grid.face_w[f] : 1.0f;   // density weight of the face
-            if (mode == 1) r2.x = wf * sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+            if (mode == 1) r2 = make_float4(wf * sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]), 0.f, 0.f, 0.f);
             else r2 = make_float4(wf * m[0], wf * m[1], wf * m[2], 0.f);
             // longest edge of the triangle (squared) and the sum of its squared edges
             const float c[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]};
@@ -93,6 +95,7 @@ __global__ void dm_k_strip_geometry(const float* __restrict__ vertices, const in
                         c2 = c[0] * c[0] + c[1] * c[1] + c[2] * c[2];
             h2 = fmaxf(fmaxf(a2, b2), c2);
             e2sum = a2 + b2 + c2;
+            r2.w = h2;   // longest squared edge of the face: a face that is coarse for the grid skips the fast path
         }
         rec[3 * (size_t)i + 0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), (float)cs);
         rec[3 * (size_t)i + 1] = make_float4((float)(-sn), e[0], e[1], e[2]);
@@ -166,7 +169,8 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
     // meshes whose edges are a few voxels long (the benchmark configurations), larger on coarse meshes.
     // One value per thread, taken at the largest |k| of its run.
     const float kye = fmaxf(fabsf(grid.kstep[1] * (float)nys0), fabsf(grid.kstep[1] * (float)(nys0 + DM_K - 1)));
-    const float kh2 = 0.01f * (kx * kx + kye * kye + kz * kz) * hmean2;   // (|k| h_rms / 10)^2
+    const float k2t = kx * kx + kye * kye + kz * kz;          // largest |k|^2 of the thread's run
+    const float kh2 = 0.01f * k2t * hmean2;                   // (|k| h_rms / 10)^2
     const float tau_t = tau * fmaxf(1.0f, kh2 * sqrtf(kh2));
     bool live = false;
 #pragma unroll
@@ -206,9 +210,13 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                                                           __float_as_uint(r0.z)));
                 const cf rho = {r0.w, r1.x};
                 const float gxz = dm_edge_gxz(kx, kz, r1.y, r1.w);
+                // a face that is coarse for this frequency (|k| h_T > 19: the error of the fast form would be > 4x the
+                // calibrated one) contributes nothing here and goes to the robust branches whole
+                const bool force = k2t * r2.w > DM_FORCE_KH2;
+                const float r2x = force ? 0.f : r2.x, r2y = force ? 0.f : r2.y;
                 float mxz = 0.f;
-                if (MODE == 0) mxz = fmaf(kx, r2.x, kz * r2.z);
-                bool any_bad = false;
+                if (MODE == 0) mxz = force ? 0.f : fmaf(kx, r2.x, kz * r2.z);
+                bool any_bad = force;
 #pragma unroll
                 for (int j = 0; j < DM_K; ++j) {
                     const float dn = dm_edge_gap(kyj[j], r1.z, gxz);
@@ -216,7 +224,7 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                     const float pr = dm_gap_product(dp[j], dn, df);
                     const bool bad = fabsf(pr) < tauj[j];
                     any_bad |= bad;
-                    float sc = (MODE == 1) ? r2.x : fmaf(kyj[j], r2.y, mxz);
+                    float sc = (MODE == 1) ? r2x : fmaf(kyj[j], r2y, mxz);
                     sc = bad ? 0.f : sc * dm_rcp_ftz(pr);
                     // nodes x0 = v_ret, x1 = v_prev, x2 = v_new; gaps p = dp, r = dn, q = df:
                     //   c0 = -r/(pqr), c1 = +q/(pqr), c2 = -p/(pqr)
@@ -252,12 +260,13 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                     if (!valid) continue;
                     const float4 r0 = tile[3 * (s + 1)], r1 = tile[3 * (s + 1) + 1], q1 = tile[3 * s + 1];
                     const float gn = dm_edge_gxz(kx, kz, r1.y, r1.w), gp = dm_edge_gxz(kx, kz, q1.y, q1.w);
+                    const bool force = k2t * r2.w > DM_FORCE_KH2;   // the whole record was left to this path
                     uint32_t mask = 0;
 #pragma unroll
                     for (int j = 0; j < DM_K; ++j) {
                         float df;
                         const float pr = dm_gap_product(dm_edge_gap(kyj[j], q1.z, gp), dm_edge_gap(kyj[j], r1.z, gn), df);
-                        mask |= (fabsf(pr) < tauj[j] ? 1u : 0u) << j;
+                        mask |= (((force && tauj[j] >= 0.f) || fabsf(pr) < tauj[j]) ? 1u : 0u) << j;
                     }
                     while (mask) {
                         const int j = __ffs(mask) - 1;
