@@ -34,6 +34,8 @@ static_assert(DM_STRIP_UNROLL == 6, "the strip loop is unrolled by 6 (window per
 #define DM_FAST_TILE 384            // strip records per shared-memory tile (multiple of DM_STRIP_UNROLL and of 32)
 #endif
 #define DM_FORCE_KH2 361.0f          // (|k| h_T)^2 above which a face skips the fast path of the forward kernel
+#define DM_FORCE_OUTLIER_KH2 64.0f   // the same for a face whose longest edge is an outlier of the mesh:
+#define DM_FORCE_OUTLIER_RATIO2 6.25f //   h_T^2 > 6.25 h_rms^2
 #define DM_LOWK_RADIUS 0.5f         // |k| h_max below which a frequency is "low" (all gaps small for all triangles)
 #define DM_LOWK_BOX 24              // low-k kernel covers |n_a| <= DM_LOWK_BOX
 
@@ -171,7 +173,16 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
     const float kye = fmaxf(fabsf(grid.kstep[1] * (float)nys0), fabsf(grid.kstep[1] * (float)(nys0 + DM_K - 1)));
     const float k2t = kx * kx + kye * kye + kz * kz;          // largest |k|^2 of the thread's run
     const float kh2 = 0.01f * k2t * hmean2;                   // (|k| h_rms / 10)^2
-    const float tau_t = tau * fmaxf(1.0f, kh2 * sqrtf(kh2));
+    // A mesh whose longest edge is far above its RMS edge (stretched meshes, outlier faces) shrinks the ball the low-k
+    // kernel owns (|k| h_max < DM_LOWK_RADIUS), so this kernel meets frequencies at which most faces have three small
+    // gaps: the threshold grows with h_max / h_rms - 1.5, between 1 (h_max <= 2.5 h_rms: the benchmark meshes) and 16.
+    const float ar = fminf(fmaxf(sqrtf(hmax2 / fmaxf(hmean2, 1e-30f)) - 1.5f, 1.0f), 16.0f);
+    const float tau_t = tau * ar * fmaxf(1.0f, kh2 * sqrtf(kh2));
+    // Longest squared edge above which a face skips the fast path at this thread's frequencies: |k| h_T > 19 for any
+    // face, |k| h_T > 8 already for a face that is an outlier of its mesh (h_T > 2.5 h_rms: none on the benchmark meshes).
+    // Such a face can have one gap of the order of its own rounding error while |pqr| is still far above tau.
+    const float ik2t = 1.0f / fmaxf(k2t, 1e-30f);
+    const float force_h2 = fminf(DM_FORCE_KH2 * ik2t, fmaxf(DM_FORCE_OUTLIER_KH2 * ik2t, DM_FORCE_OUTLIER_RATIO2 * hmean2));
     bool live = false;
 #pragma unroll
     for (int j = 0; j < DM_K; ++j) {
@@ -210,9 +221,9 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                                                           __float_as_uint(r0.z)));
                 const cf rho = {r0.w, r1.x};
                 const float gxz = dm_edge_gxz(kx, kz, r1.y, r1.w);
-                // a face that is coarse for this frequency (|k| h_T > 19: the error of the fast form would be > 4x the
-                // calibrated one) contributes nothing here and goes to the robust branches whole
-                const bool force = k2t * r2.w > DM_FORCE_KH2;
+                // a face that is coarse for this frequency (h_T^2 > force_h2 above) contributes
+                // nothing here and goes to the robust branches whole
+                const bool force = r2.w > force_h2;
                 const float r2x = force ? 0.f : r2.x, r2y = force ? 0.f : r2.y;
                 float mxz = 0.f;
                 if (MODE == 0) mxz = force ? 0.f : fmaf(kx, r2.x, kz * r2.z);
@@ -260,7 +271,7 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                     if (!valid) continue;
                     const float4 r0 = tile[3 * (s + 1)], r1 = tile[3 * (s + 1) + 1], q1 = tile[3 * s + 1];
                     const float gn = dm_edge_gxz(kx, kz, r1.y, r1.w), gp = dm_edge_gxz(kx, kz, q1.y, q1.w);
-                    const bool force = k2t * r2.w > DM_FORCE_KH2;   // the whole record was left to this path
+                    const bool force = r2.w > force_h2;   // the whole record was left to this path
                     uint32_t mask = 0;
 #pragma unroll
                     for (int j = 0; j < DM_K; ++j) {

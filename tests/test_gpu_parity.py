@@ -444,3 +444,38 @@ def test_coarse_meshes_large_gaps(dm, mode):
         dref = oracle.mesh_ft_backward_grid(v, f, n, spacing, mode, G.astype(np.complex128))
         assert _rel_l2(dv, dref) <= GRAD_TOL, (len(f), _rel_l2(dv, dref))
         plan.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_stretched_meshes_and_outlier_faces(dm, mode):
+    """Anisotropically scaled meshes (aspect ratio up to 6) with a second, much finer or coarser component: the longest
+    edge is several times the RMS edge, so the low-k kernel's ball shrinks and single faces are coarse for frequencies
+    at which the mesh as a whole is not ("Stretched meshes and outlier faces")."""
+    import torch
+    from workloads.meshes import perturb_radial
+    rng = np.random.default_rng(73)
+    cases = []
+    c = np.array([-0.08, 0.02, 0.05])
+    v, f = icosphere(3, 0.3, c)
+    v = c + (perturb_radial(v, c, 0.08, rng) - c) * np.array([0.9, 0.2, 1.3])
+    v2, f2 = icosphere(1, 0.2, (0.02, 0.1, -0.2))
+    v2 = v2 * np.array([0.3, 1.4, 1.0])
+    cases.append((np.vstack([v, v2]), np.vstack([f, f2 + len(v)]), (33, 18, 16), (1.13, 1.66, 1.09)))
+    c = np.array([0.05, 0.1, 0.06])
+    v, f = icosphere(1, 0.42, c)
+    v = c + (perturb_radial(v, c, 0.08, rng) - c) * np.array([1.25, 1.5, 1.4])
+    v2, f2 = icosphere(2, 0.1, (-0.3, -0.35, -0.3))
+    cases.append((np.vstack([v, v2]), np.vstack([f, f2 + len(v)]), (36, 34, 28), (1.58, 1.99, 1.72)))
+    for v, f, n, L in cases:
+        v, f = v.astype(np.float32), f.astype(np.int32)
+        spacing = tuple(np.array(L) / np.array(n))
+        origin = tuple(-np.array(L) / 2 + 0.3 * np.array(spacing))
+        plan = dm.Plan(n, spacing, origin, mode, torch.as_tensor(f, device="cuda"), v.shape[0])
+        F = plan.mesh_ft_forward(_dev(v)).cpu().numpy()
+        ref = oracle.mesh_ft_forward_grid(v, f, n, spacing, mode)
+        assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0]), (len(f), np.abs(F - ref).max() / abs(ref[0, 0, 0]))
+        G = (rng.standard_normal(ref.shape) + 1j * rng.standard_normal(ref.shape)).astype(np.complex64)
+        dv = plan.mesh_ft_backward(_dev(v), _dev(G)).cpu().numpy()
+        dref = oracle.mesh_ft_backward_grid(v, f, n, spacing, mode, G.astype(np.complex128))
+        assert _rel_l2(dv, dref) <= GRAD_TOL, (len(f), _rel_l2(dv, dref))
+        plan.close()
