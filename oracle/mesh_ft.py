@@ -190,6 +190,9 @@ def mesh_ft_forward_weighted(vertices, faces, kvec, mode: int, weights) -> np.nd
 
 
 def mesh_ft_backward_weighted(vertices, faces, kvec, mode: int, G, weights) -> np.ndarray:
+    """dL/dv of mesh_ft_forward_weighted, by the same linearity over the groups of equal weight.  Pinned by central
+    finite differences of the weighted forward, the translation identity and a per-corner assembly that never groups
+    faces (tests/test_oracle_backward.py::test_weighted_backward_*)."""
     v = np.asarray(vertices, dtype=np.float64).reshape(-1, 3)
     out = np.zeros_like(v)
     for u, fg in _weight_groups(faces, weights):

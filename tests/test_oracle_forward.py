@@ -190,3 +190,45 @@ def test_per_face_weights_are_linear_in_the_density():
         assert np.abs(got - want).max() <= 1e-13 * abs(want[0])
     vol = lambda vv, ff: np.einsum("ij,ij->i", vv[ff[:, 0]], np.cross(vv[ff[:, 1]], vv[ff[:, 2]])).sum() / 6.0
     assert abs(oracle.mesh_ft_forward_weighted(v, f, k[:1], VOL, w)[0] - (vol(vo, fo) - 0.5 * vol(vi, fi))) < 1e-14
+
+
+def test_weighted_surface_forward_vs_gauss_quadrature():
+    """Independent pin of oracle.mesh_ft_forward_weighted away from k = 0 (not its own linearity): per-face weights
+    w_T times the tensor Gauss-Legendre quadrature of int_T e^{-ik.x} dS, three distinct weights incl. a negative one,
+    assigned per face at random (reading R23)."""
+    rng = np.random.default_rng(31)
+    v, f = icosphere(1, 0.35, (0.02, 0.01, -0.03))
+    v = perturb_radial(v, (0.02, 0.01, -0.03), 0.12, rng)
+    wts = rng.choice([1.0, 0.4, -0.7], size=len(f))
+    k = rng.uniform(-14, 14, (30, 3))
+    x, w = np.polynomial.legendre.leggauss(32)
+    x, w = 0.5 * (x + 1), 0.5 * w
+    U, W = np.meshgrid(x, x, indexing="ij")
+    wt = np.outer(w, w) * (1 - U)
+    ref = np.zeros(len(k), dtype=complex)
+    for t, tri in enumerate(f):
+        p0, p1, p2 = v[tri]
+        pts = p0 + U[..., None] * (p1 - p0) + (W * (1 - U))[..., None] * (p2 - p0)
+        twoA = np.linalg.norm(np.cross(p1 - p0, p2 - p0))
+        ref += wts[t] * twoA * np.einsum("ij,ijq->q", wt, np.exp(-1j * np.einsum("ijd,qd->ijq", pts, k)))
+    got = oracle.mesh_ft_forward_weighted(v, f, k, SURF, wts)
+    assert np.abs(got - ref).max() < 1e-12
+
+
+def test_weighted_volume_forward_vs_per_face_divergence_terms():
+    """Volume mode with per-face weights, away from k = 0: F_w(k) = (i/|k|^2) sum_T w_T (k.m_T) f_T(k) assembled face
+    by face from one-triangle calls of the SURFACE-mode oracle (2 A_T f_T = the one-face surface FT, pinned by
+    quadrature above), so neither the volume-mode code path nor the weight grouping is reused."""
+    rng = np.random.default_rng(33)
+    v, f = icosphere(1, 0.3, (-0.02, 0.03, 0.01))
+    v = perturb_radial(v, (-0.02, 0.03, 0.01), 0.1, rng)
+    wts = rng.choice([1.0, 0.5, -0.8], size=len(f))
+    k = rng.uniform(-25, 25, (16, 3))
+    want = np.zeros(len(k), dtype=complex)
+    for t, tri in enumerate(f):
+        p0, p1, p2 = v[tri]
+        m = np.cross(p1 - p0, p2 - p0)
+        surf = oracle.mesh_ft_forward(v, f[t:t + 1], k, SURF)          # |m_T| f_T(k)
+        want += wts[t] * 1j * (k @ m) / np.linalg.norm(m) * surf / (k * k).sum(axis=1)
+    got = oracle.mesh_ft_forward_weighted(v, f, k, VOL, wts)
+    assert np.abs(got - want).max() < 1e-12 * np.abs(want).max()
