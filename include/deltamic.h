@@ -89,7 +89,8 @@ int dm_plan_set_face_weights(dm_plan* plan, const float* weights_dev);
  * exp(-1/2 k^T B k) > cutoff: dm_mesh_ft_forward writes 0 everywhere else, dm_mesh_ft_backward ignores dL/dF there
  * (the gradient of the banded forward).  dm_render* use the band too; B is normally the PSF they are called with.
  * psf_cov_host = NULL switches the band off (the default).  k = 0 is always inside the band.  Setting the band
- * synchronises the stream (it builds the list of active frequencies). */
+ * synchronises the stream (it builds the list of active frequencies).  A call that fails leaves the plan's previous
+ * band (or no band) in force. */
 int dm_plan_set_narrow_band(dm_plan* plan, const float* psf_cov_host, float cutoff);
 
 /* Tuning / debugging knobs.  Defaults are the product path; the "robust" paths evaluate EVERY pair through the
@@ -97,7 +98,7 @@ int dm_plan_set_narrow_band(dm_plan* plan, const float* psf_cov_host, float cuto
 typedef enum dm_option {
     DM_OPT_FORWARD_PATH  = 0, /* 0 = fast strip kernel (default), 1 = robust per-triangle kernel                  */
     DM_OPT_BACKWARD_PATH = 1, /* 0 = fast kernel (default), 1 = robust kernel                                     */
-    DM_OPT_TAU           = 2, /* forward: gap-product threshold |pqr| below which a pair leaves the fast path       */
+    DM_OPT_TAU           = 2, /* forward: gap-product threshold |pqr| at or below which a pair leaves the fast path (>= 0) */
     DM_OPT_TAU_BWD       = 3, /* backward: threshold on m1^2 m2 (the two smallest |gaps|) below which a pair leaves
                                  the fast path                                                                     */
     DM_OPT_AREA_NORMALISED = 4 /* DM_SURFACE only; 1 = the paper's membrane density u = F / |Lambda| (PAPER.md:177-186
@@ -159,6 +160,11 @@ int dm_plan_stage_ms(dm_plan* plan, float ms[4]);
 
 /* Number of CUDA kernels (cuFFT's excluded) the plan has launched since creation. */
 int64_t dm_plan_launch_count(const dm_plan* plan);
+
+/* Which kernels the LAST forward / backward mesh FT of this plan ran: paths[0] forward, paths[1] backward;
+ * 0 = fast kernels, 1 = robust kernels (every pair through the series / far-pair branches: DM_OPT_*_PATH = 1, or a
+ * weight set outside the fast kernels' validated regime), -1 = no such call yet.  Host-side bookkeeping, no sync. */
+int dm_plan_paths_used(const dm_plan* plan, int32_t paths[2]);
 
 void dm_plan_destroy(dm_plan* plan);
 

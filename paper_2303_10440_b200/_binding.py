@@ -14,7 +14,7 @@ DM_OPT_FORWARD_PATH, DM_OPT_BACKWARD_PATH, DM_OPT_TAU, DM_OPT_TAU_BWD, DM_OPT_AR
 _SYMBOLS = (
     "dm_plan_create", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_render",
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
-    "dm_plan_launch_count", "dm_plan_destroy", "dm_error_string", "dm_version",
+    "dm_plan_launch_count", "dm_plan_paths_used", "dm_plan_destroy", "dm_error_string", "dm_version",
 )
 
 
@@ -65,6 +65,7 @@ def load_library():
     lib.dm_plan_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     lib.dm_plan_launch_count.argtypes = [vp]
     lib.dm_plan_launch_count.restype = ctypes.c_int64
+    lib.dm_plan_paths_used.argtypes = [vp, ctypes.POINTER(ctypes.c_int32)]
     lib.dm_plan_destroy.argtypes = [vp]
     lib.dm_plan_destroy.restype = None
     lib.dm_error_string.argtypes = [ctypes.c_int]
@@ -238,6 +239,12 @@ class Plan:
 
     def launch_count(self) -> int:
         return int(self._lib.dm_plan_launch_count(self._h))
+
+    def paths_used(self):
+        """(forward, backward) kernels of the last mesh-FT calls: 0 = fast, 1 = robust, -1 = not called yet."""
+        out = (ctypes.c_int32 * 2)()
+        _check(self._lib.dm_plan_paths_used(self._h, out), "dm_plan_paths_used")
+        return int(out[0]), int(out[1])
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

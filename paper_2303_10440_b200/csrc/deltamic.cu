@@ -52,6 +52,11 @@ struct dm_plan {
     double* dc_total = nullptr;      // [1] fp64 volume / total area of the last forward (k = 0 kernels)
     double* dot_part = nullptr;      // [DM_DOT_BLOCKS + 1] block sums and result of sum_k Re(conj(G) F)
     float* face_w = nullptr;         // [n_faces] per-face density weights, valid while gd.face_w points at it
+    bool weights_robust = false;     // the weights are outside the regime the fast kernels are validated for (mixed
+                                     // sign, or varying inside a connected component in volume mode): every pair goes
+                                     // through the robust kernels
+    std::vector<int32_t> face_comp;  // host: connected component (shared vertices) of every face, built at create
+    int last_fwd_path = -1, last_bwd_path = -1;   // 0 = fast, 1 = robust: what the last mesh-FT calls actually ran
     long long band_count = 0;        // stored frequencies inside the narrow band (whole grid)
     uint32_t* band_slots = nullptr;  // the forward kernel's thread list under the narrow band
     int2* band_z = nullptr;          // [nx*ny] in-band z interval of every row (narrow band), valid while band_on
@@ -218,7 +223,9 @@ int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
 
 int run_forward_raw(dm_plan* p, const float* vertices_dev, float* F_dev)
 {
-    int rc = p->fwd_path == 0 ? run_forward_fast(p, vertices_dev, F_dev) : run_forward_robust(p, vertices_dev, F_dev);
+    const bool robust = p->fwd_path != 0 || p->weights_robust;
+    p->last_fwd_path = robust ? 1 : 0;
+    int rc = robust ? run_forward_robust(p, vertices_dev, F_dev) : run_forward_fast(p, vertices_dev, F_dev);
     if (rc) return rc;
     if (p->ix_begin == 0) {
         dm_k_dc_partial<<<DM_DC_BLOCKS, 256, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode, p->gd.face_w, p->dc_part);
@@ -242,6 +249,7 @@ int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
 
 int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, float* dv_dev)
 {
+    if (p->normalise && (p->ix_begin != 0 || p->ix_end != p->gd.nx)) return DM_ERR_UNSUPPORTED;   // before any launch
     int rps = 1;
     const int n_split = backward_splits(p, &rps);
     dim3 grid((p->n_faces + 127) / 128, n_split);
@@ -260,7 +268,9 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     const size_t row_smem = 2 * (size_t)nzh * sizeof(float4) + (size_t)n_seed * DM_BF_THREADS * sizeof(float2) +
                             (size_t)(DM_BF_THREADS / 32) * DM_BF_STAGE * DM_PATCH_MAXV * sizeof(float2);
     int rc;
-    if (p->bwd_path == 0 && nzh <= 288) {
+    const bool robust = p->bwd_path != 0 || p->weights_robust || nzh > 288;
+    p->last_bwd_path = robust ? 1 : 0;
+    if (!robust) {
         const DmPatchDev pt = {p->pt_face, p->pt_vid, p->pt_loc, p->pt_lanes};
         grid.x = (unsigned)(p->pt_lanes / DM_BF_THREADS);
         if (cudaMemsetAsync(p->hmax2, 0, 16, p->stream) != cudaSuccess) return DM_ERR_CUDA;
@@ -298,7 +308,6 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     const double *area_total = nullptr, *sdot = nullptr;
     if (p->normalise) {
         // eq. 13's second term needs |Lambda| and sum_k Re(conj(G) F): one raw forward of these vertices and a dot product
-        if (p->ix_begin != 0 || p->ix_end != p->gd.nx) return DM_ERR_UNSUPPORTED;
         const long long nk = (long long)n_k_of(p);
         if (!p->spec3 && cudaMalloc(&p->spec3, (size_t)nk * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
         if (!p->dot_part && cudaMalloc(&p->dot_part, (DM_DOT_BLOCKS + 1) * sizeof(double)) != cudaSuccess) return DM_ERR_ALLOC;
@@ -442,6 +451,28 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
         try { fill.assign(off.begin(), off.end() - 1); } catch (...) { rc = DM_ERR_ALLOC; break; }
         for (size_t i = 0; i < faces_h.size(); ++i) cor[(size_t)fill[faces_h[i]]++] = (int32_t)i;
 
+        // connected components of the faces (shared vertices; union-find), used to classify per-face weights
+        try {
+            std::vector<int32_t> parent((size_t)n_vertices);
+            for (int32_t v = 0; v < n_vertices; ++v) parent[v] = v;
+            auto find = [&](int32_t a) {
+                while (parent[a] != a) {
+                    parent[a] = parent[parent[a]];
+                    a = parent[a];
+                }
+                return a;
+            };
+            for (int32_t t = 0; t < n_faces; ++t) {
+                const int32_t a = find(faces_h[3 * (size_t)t]);
+                for (int j = 1; j < 3; ++j) {
+                    const int32_t b = find(faces_h[3 * (size_t)t + j]);
+                    if (b != a) parent[b] = a;
+                }
+            }
+            p->face_comp.resize((size_t)n_faces);
+            for (int32_t t = 0; t < n_faces; ++t) p->face_comp[t] = find(faces_h[3 * (size_t)t]);
+        } catch (...) { rc = DM_ERR_ALLOC; break; }
+
         const size_t nk = n_k_of(p);
         // k-splits of the backward: a small mesh has few triangle blocks, so it needs many splits to fill the machine
         // (up to 48 CTAs per SM slot), within 64 M floats of partial sums
@@ -541,13 +572,49 @@ int dm_plan_set_face_weights(dm_plan* p, const float* weights_dev)
     if (!p) return DM_ERR_INVALID_ARG;
     if (!weights_dev) {
         p->gd.face_w = nullptr;
+        p->weights_robust = false;
         return DM_OK;
+    }
+    // classify on the host (this call synchronises the stream): the fast kernels' flag thresholds are validated, against
+    // the tolerance 1e-4 |F(0)|, for weights of one sign that -- in volume mode -- are constant on every connected
+    // component (regions of different density); anything else (mixed signs: F(0) cancels and stops being the scale of the
+    // spectrum; weights varying inside a component in volume mode: the rounding errors of a shared edge no longer cancel
+    // between its two faces) is evaluated pair by pair through the robust branches
+    std::vector<float> wh;
+    try { wh.resize((size_t)p->n_faces); } catch (...) { return DM_ERR_ALLOC; }
+    if (cudaMemcpyAsync(wh.data(), weights_dev, wh.size() * sizeof(float), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+        cudaStreamSynchronize(p->stream) != cudaSuccess)
+        return DM_ERR_CUDA;
+    bool pos = false, neg = false, split = false;
+    std::vector<float> comp_w;
+    std::vector<char> comp_seen;
+    try {
+        if (p->mode == DM_VOLUME) {
+            comp_w.assign((size_t)p->n_vertices, 0.f);
+            comp_seen.assign((size_t)p->n_vertices, 0);
+        }
+    } catch (...) { return DM_ERR_ALLOC; }
+    for (int32_t t = 0; t < p->n_faces; ++t) {
+        const float w = wh[t];
+        if (!std::isfinite(w)) return DM_ERR_INVALID_ARG;
+        pos = pos || w > 0.f;
+        neg = neg || w < 0.f;
+        if (p->mode == DM_VOLUME) {
+            const int32_t c = p->face_comp[t];
+            if (!comp_seen[c]) {
+                comp_seen[c] = 1;
+                comp_w[c] = w;
+            } else if (comp_w[c] != w) {
+                split = true;
+            }
+        }
     }
     if (!p->face_w && cudaMalloc(&p->face_w, (size_t)p->n_faces * sizeof(float)) != cudaSuccess) return DM_ERR_ALLOC;
     if (cudaMemcpyAsync(p->face_w, weights_dev, (size_t)p->n_faces * sizeof(float), cudaMemcpyDeviceToDevice, p->stream) !=
         cudaSuccess)
         return DM_ERR_CUDA;
     p->gd.face_w = p->face_w;
+    p->weights_robust = (pos && neg) || split;
     return DM_OK;
 }
 
@@ -565,10 +632,10 @@ int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
     if (!(cutoff > 0.f) || !(cutoff < 1.f)) return DM_ERR_INVALID_ARG;
     for (int i = 0; i < 6; ++i)
         if (!std::isfinite(psf_cov_host[i])) return DM_ERR_INVALID_ARG;
-    if (!p->band_z && cudaMalloc(&p->band_z, (size_t)p->gd.nx * p->gd.ny * sizeof(int2)) != cudaSuccess) return DM_ERR_ALLOC;
-    for (int i = 0; i < 6; ++i) p->gd.band_cov[i] = psf_cov_host[i];
-    p->gd.band_lim = std::log(1.0f / cutoff);
-    p->band_on = true;
+    // Everything is built beside the plan's current band and committed at the end: a failed call leaves the plan as it was.
+    DmGridDev g = p->gd;
+    for (int i = 0; i < 6; ++i) g.band_cov[i] = psf_cov_host[i];
+    g.band_lim = std::log(1.0f / cutoff);
     // extent of the band ellipsoid along z: k_z^2 <= 2 L (B^-1)_zz; two frequencies of margin, the whole axis when B is
     // not positive definite
     {
@@ -576,60 +643,73 @@ int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
                      xz = psf_cov_host[4], yz = psf_cov_host[5];
         const double det = xx * (yy * zz - yz * yz) - xy * (xy * zz - yz * xz) + xz * (xy * yz - yy * xz);
         const double cof = xx * yy - xy * xy;
-        p->gd.nzb = p->gd.nzh;
+        g.nzb = g.nzh;
         if (det > 0.0 && cof > 0.0 && xx > 0.0) {
-            const double kz_max = std::sqrt(2.0 * (double)p->gd.band_lim * cof / det);
-            const double nz_max = kz_max / (double)p->gd.kstep[2];
-            if (nz_max + 3.0 < (double)p->gd.nzh) p->gd.nzb = (int)nz_max + 3;
+            const double kz_max = std::sqrt(2.0 * (double)g.band_lim * cof / det);
+            const double nz_max = kz_max / (double)g.kstep[2];
+            if (nz_max + 3.0 < (double)g.nzh) g.nzb = (int)nz_max + 3;
         }
     }
-    const int n_rows = p->gd.nx * p->gd.ny;
-    p->gd.band_slots = nullptr;   // the row intervals are computed with the band test alone
-    p->gd.n_band_slots = 0;
-    dm_k_band_rows<<<(n_rows + 127) / 128, 128, 0, p->stream>>>(p->gd, p->band_z);
-    int rc = check_launch(p);
-    if (rc) return rc;
-    // the forward kernel's thread list: every (i_x, run of DM_K signed y-frequencies, i_z) with a frequency in the band
+    const int n_rows = g.nx * g.ny;
+    g.band_slots = nullptr;   // the row intervals are computed with the band test alone
+    g.n_band_slots = 0;
+    int2* band_z_new = nullptr;
+    uint32_t* slots_new = nullptr;
+    int rc = DM_OK;
+    long long count = 0;
     std::vector<int2> bz;
     std::vector<uint32_t> slots;
-    try {
-        bz.resize((size_t)n_rows);
-    } catch (...) { return DM_ERR_ALLOC; }
-    if (cudaMemcpyAsync(bz.data(), p->band_z, (size_t)n_rows * sizeof(int2), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
-        cudaStreamSynchronize(p->stream) != cudaSuccess)
-        return DM_ERR_CUDA;
-    p->band_count = 0;
-    for (const int2& b : bz) p->band_count += std::max(0, b.y - b.x);
-    const int ny = p->gd.ny, n_yruns = (ny + DM_K - 1) / DM_K;
-    if (p->gd.nx <= 4096 && n_yruns <= 2048 && p->gd.nzh <= 512) {
-        try {
-            for (int ix = 0; ix < p->gd.nx; ++ix)
-                for (int yrun = 0; yrun < n_yruns; ++yrun) {
-                    int lo = p->gd.nzh, hi = 0;
-                    for (int j = 0; j < DM_K; ++j) {
-                        const int nys = -(ny / 2) + yrun * DM_K + j;
-                        if (nys > (ny - 1) / 2) break;
-                        const int2 b = bz[(size_t)ix * ny + (nys < 0 ? nys + ny : nys)];
-                        if (b.y > b.x) {
-                            lo = std::min(lo, b.x);
-                            hi = std::max(hi, b.y);
+    do {
+        if (cudaMalloc(&band_z_new, (size_t)n_rows * sizeof(int2)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
+        dm_k_band_rows<<<(n_rows + 127) / 128, 128, 0, p->stream>>>(g, band_z_new);
+        if ((rc = check_launch(p))) break;
+        // the forward kernel's thread list: every (i_x, run of DM_K signed y-frequencies, i_z) with a frequency in the band
+        try { bz.resize((size_t)n_rows); } catch (...) { rc = DM_ERR_ALLOC; break; }
+        if (cudaMemcpyAsync(bz.data(), band_z_new, (size_t)n_rows * sizeof(int2), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+            cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+        for (const int2& b : bz) count += std::max(0, b.y - b.x);
+        const int ny = g.ny, n_yruns = (ny + DM_K - 1) / DM_K;
+        if (g.nx <= 4096 && n_yruns <= 2048 && g.nzh <= 512) {
+            try {
+                for (int ix = 0; ix < g.nx; ++ix)
+                    for (int yrun = 0; yrun < n_yruns; ++yrun) {
+                        int lo = g.nzh, hi = 0;
+                        for (int j = 0; j < DM_K; ++j) {
+                            const int nys = -(ny / 2) + yrun * DM_K + j;
+                            if (nys > (ny - 1) / 2) break;
+                            const int2 b = bz[(size_t)ix * ny + (nys < 0 ? nys + ny : nys)];
+                            if (b.y > b.x) {
+                                lo = std::min(lo, b.x);
+                                hi = std::max(hi, b.y);
+                            }
                         }
+                        for (int iz = lo; iz < hi; ++iz) slots.push_back(((uint32_t)ix << 20) | ((uint32_t)yrun << 9) | (uint32_t)iz);
                     }
-                    for (int iz = lo; iz < hi; ++iz) slots.push_back(((uint32_t)ix << 20) | ((uint32_t)yrun << 9) | (uint32_t)iz);
-                }
-        } catch (...) { return DM_ERR_ALLOC; }
-        if (!slots.empty()) {
-            cudaFree(p->band_slots);
-            p->band_slots = nullptr;
-            if (cudaMalloc(&p->band_slots, slots.size() * sizeof(uint32_t)) != cudaSuccess) return DM_ERR_ALLOC;
-            if (cudaMemcpyAsync(p->band_slots, slots.data(), slots.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, p->stream) !=
-                    cudaSuccess ||
-                cudaStreamSynchronize(p->stream) != cudaSuccess)
-                return DM_ERR_CUDA;
-            p->gd.band_slots = p->band_slots;
-            p->gd.n_band_slots = (int)slots.size();
+            } catch (...) { rc = DM_ERR_ALLOC; break; }
+            if (!slots.empty()) {
+                if (cudaMalloc(&slots_new, slots.size() * sizeof(uint32_t)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
+                if (cudaMemcpyAsync(slots_new, slots.data(), slots.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, p->stream) !=
+                        cudaSuccess ||
+                    cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+                g.band_slots = slots_new;
+                g.n_band_slots = (int)slots.size();
+            }
         }
+    } while (0);
+    if (rc != DM_OK) {
+        cudaFree(band_z_new);
+        cudaFree(slots_new);
+        cudaGetLastError();
+        return rc;
     }
+    // commit (the stream is idle: the copies above were synchronised)
+    cudaFree(p->band_z);
+    cudaFree(p->band_slots);
+    p->band_z = band_z_new;
+    p->band_slots = slots_new;
+    p->gd = g;
+    p->band_count = count;
+    p->band_on = true;
     return DM_OK;
 }
 
@@ -645,7 +725,7 @@ int dm_plan_set_option(dm_plan* p, int option, double value)
             if (value != 0.0 && value != 1.0) return DM_ERR_INVALID_ARG;
             p->bwd_path = (int)value;
             return DM_OK;
-        case DM_OPT_TAU:
+        case DM_OPT_TAU:      // 0 is allowed: only exactly vanishing gap products then leave the fast path
             if (!(value >= 0.0) || !std::isfinite(value)) return DM_ERR_INVALID_ARG;
             p->tau = (float)value;
             return DM_OK;
@@ -763,6 +843,14 @@ int dm_plan_stage_ms(dm_plan* p, float ms[4])
 }
 
 int64_t dm_plan_launch_count(const dm_plan* p) { return p ? p->launches : 0; }
+
+int dm_plan_paths_used(const dm_plan* p, int32_t paths[2])
+{
+    if (!p || !paths) return DM_ERR_INVALID_ARG;
+    paths[0] = p->last_fwd_path;
+    paths[1] = p->last_bwd_path;
+    return DM_OK;
+}
 
 void dm_plan_destroy(dm_plan* p)
 {

@@ -233,7 +233,7 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                     const float dn = dm_edge_gap(kyj[j], r1.z, gxz);
                     float df;
                     const float pr = dm_gap_product(dp[j], dn, df);
-                    const bool bad = fabsf(pr) < tauj[j];
+                    const bool bad = !(fabsf(pr) > tauj[j]);   // also catches pr = 0 when tau = 0 (0 * rcp(0) would be NaN)
                     any_bad |= bad;
                     float sc = (MODE == 1) ? r2x : fmaf(kyj[j], r2y, mxz);
                     sc = bad ? 0.f : sc * dm_rcp_ftz(pr);
@@ -277,7 +277,7 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                     for (int j = 0; j < DM_K; ++j) {
                         float df;
                         const float pr = dm_gap_product(dm_edge_gap(kyj[j], q1.z, gp), dm_edge_gap(kyj[j], r1.z, gn), df);
-                        mask |= (((force && tauj[j] >= 0.f) || fabsf(pr) < tauj[j]) ? 1u : 0u) << j;
+                        mask |= (((force && tauj[j] >= 0.f) || !(fabsf(pr) > tauj[j])) ? 1u : 0u) << j;
                     }
                     while (mask) {
                         const int j = __ffs(mask) - 1;
