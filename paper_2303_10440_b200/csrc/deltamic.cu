@@ -61,6 +61,7 @@ struct dm_plan {
     uint32_t* band_slots = nullptr;  // the forward kernel's thread list under the narrow band
     int2* band_z = nullptr;          // [nx*ny] in-band z interval of every row (narrow band), valid while band_on
     bool band_on = false;
+    float2* kappa = nullptr;         // [n_k] kappa(k) of the fast backward kernel (dm_k_kappa), allocated on first use
     float2* spec3 = nullptr;         // [n_k] forward spectrum recomputed for the PSF gradient (allocated on first use)
     double* psfg_part = nullptr;     // [DM_PSFG_BLOCKS*6] block sums of the PSF gradient
     float* psfg_out = nullptr;       // [6] device result of the PSF gradient
@@ -253,8 +254,6 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     int rps = 1;
     const int n_split = backward_splits(p, &rps);
     dim3 grid((p->n_faces + 127) / 128, n_split);
-    // seed spacing of the fast kernel: the smallest SEG whose seed table (ceil(nzh/SEG)-1 entries x 128 threads x 8 B,
-    // one vertex slot per thread) has at most 8 entries per vertex
     const int nzh = p->gd.nzh;
     // The flag threshold is calibrated for sums over many frequencies (errors of single pairs average out); when a vertex
     // gradient sums fewer than ~5e4 frequencies (tiny grids, narrow bands, thin slabs) one pair just above the threshold
@@ -263,29 +262,30 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     double n_freq = (double)p->gd.nx * p->gd.ny * nzh;
     if (p->band_on) n_freq = std::max(1.0, (double)p->band_count);
     const float tau_b_eff = (float)((double)p->tau_b * std::max(1.0, std::sqrt(5.0e4 / n_freq)));
+    // seed spacing of the fast kernel (frequencies between exact phase seeds) and the seed-table entries per vertex slot;
+    // a row longer than (n_tab + 1) seg frequencies is walked in several super-segments
     const int seg = nzh <= 72 ? 8 : (nzh <= 144 ? 16 : 32);
-    const int n_seed = (nzh + seg - 1) / seg - 1;
-    const size_t row_smem = 2 * (size_t)nzh * sizeof(float4) + (size_t)n_seed * DM_BF_THREADS * sizeof(float2) +
-                            (size_t)(DM_BF_THREADS / 32) * DM_BF_STAGE * DM_PATCH_MAXV * sizeof(float2);
+    const int n_tab = std::min(DM_BF_NTAB_MAX, (nzh + seg - 1) / seg - 1);
+    const size_t tab_smem = (size_t)n_tab * DM_BF_THREADS * sizeof(float2);
     int rc;
-    const bool robust = p->bwd_path != 0 || p->weights_robust || nzh > 288;
+    const bool robust = p->bwd_path != 0 || p->weights_robust || rps > 32768;
     p->last_bwd_path = robust ? 1 : 0;
     if (!robust) {
         const DmPatchDev pt = {p->pt_face, p->pt_vid, p->pt_loc, p->pt_lanes};
         grid.x = (unsigned)(p->pt_lanes / DM_BF_THREADS);
-        if (cudaMemsetAsync(p->hmax2, 0, 16, p->stream) != cudaSuccess) return DM_ERR_CUDA;
-        dm_k_bwd_geometry<<<(p->pt_lanes + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, pt, p->gd, p->btrec, p->bvrec,
-                                                                                  p->hmax2);
+        const size_t nk = n_k_of(p);
+        if (!p->kappa && cudaMalloc(&p->kappa, nk * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
+        dm_k_bwd_geometry<<<(p->pt_lanes + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, pt, p->gd, p->btrec, p->bvrec);
+        if ((rc = check_launch(p))) return rc;
+        const long long n_slab = (long long)(p->ix_end - p->ix_begin) * p->gd.ny * nzh;
+        if (p->mode == DM_SURFACE)
+            dm_k_kappa<1><<<(unsigned)((n_slab + 255) / 256), 256, 0, p->stream>>>((const float2*)G_dev, p->gd, p->ix_begin, p->ix_end, p->kappa);
+        else
+            dm_k_kappa<0><<<(unsigned)((n_slab + 255) / 256), 256, 0, p->stream>>>((const float2*)G_dev, p->gd, p->ix_begin, p->ix_end, p->kappa);
         if ((rc = check_launch(p))) return rc;
 #define DM_LAUNCH_BF2(MODE, SEG, BAND)                                                                                   \
-    do {                                                                                                                 \
-        if (cudaFuncSetAttribute(dm_k_backward_fast<MODE, SEG, BAND>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
-                                 (int)row_smem) != cudaSuccess)                                                          \
-            return DM_ERR_CUDA;                                                                                          \
-        dm_k_backward_fast<MODE, SEG, BAND><<<grid, DM_BF_THREADS, row_smem, p->stream>>>(                               \
-            p->btrec, p->bvrec, pt, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, tau_b_eff, (const float2*)G_dev,      \
-            p->band_z, p->part);                                                                                                 \
-    } while (0)
+    dm_k_backward_fast<MODE, SEG, BAND><<<grid, DM_BF_THREADS, tab_smem, p->stream>>>(                                   \
+        p->btrec, p->bvrec, pt, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, tau_b_eff, n_tab, p->kappa, p->band_z, p->part)
 #define DM_LAUNCH_BF(MODE, SEG)                                                                                          \
     do {                                                                                                                 \
         if (p->band_on) DM_LAUNCH_BF2(MODE, SEG, true); else DM_LAUNCH_BF2(MODE, SEG, false);                            \
@@ -481,6 +481,9 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
             long long m = ((long long)p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
             m = std::min<long long>(m, (64LL << 20) / ((long long)DM_BWD_NSUM * n_faces));
             p->n_split_max = (int)std::max<long long>(64, std::min<long long>(m, 4096));
+            // the fast kernel's queue entries hold a 15-bit row index inside the split
+            const long long rows = (long long)p->gd.nx * p->gd.ny;
+            p->n_split_max = (int)std::max<long long>(p->n_split_max, (rows + 32767) / 32768);
         }
         if (cudaMalloc(&p->faces, faces_h.size() * sizeof(int32_t)) != cudaSuccess ||
             cudaMalloc(&p->csr_off, off.size() * sizeof(int32_t)) != cudaSuccess ||
@@ -886,6 +889,7 @@ void dm_plan_destroy(dm_plan* p)
     cudaFree(p->band_slots);
     cudaFree(p->band_z);
     cudaFree(p->spec3);
+    cudaFree(p->kappa);
     cudaFree(p->psfg_part);
     cudaFree(p->psfg_out);
     if (p->ev_ok)

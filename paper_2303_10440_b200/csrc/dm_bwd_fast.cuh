@@ -1,40 +1,43 @@
 // dm_bwd_fast.cuh -- optimised backward mesh-FT kernel (rows A1, A6 of the hot path), sm_100a.
 //
 // Layout.  One THREAD owns one triangle and keeps its 13 k-sums in registers; one WARP owns a compact patch of 32
-// triangles (dm_patches.h) and a CTA of four warps walks a range of (i_x,i_y) rows of the stored spectrum, innermost
-// along z.  Every thread of the CTA is at the SAME frequency at the same time, so everything that depends on k only --
-// kappa = conj(G) (surface) or i conj(G)/|k|^2 (volume), k_z -- is computed once per CTA and row into shared memory and
-// read back as one broadcast LDS.128 per pair, and there is no reduction across threads at all (O(N n_v)
-// backward; :182-186 eq. 13 is the later CSR gather).
+// triangles (dm_patches.h) and walks a range of (i_x,i_y) rows of the stored spectrum, innermost along z.  The warps of a
+// CTA are completely independent -- there is no CTA-wide barrier after the set-up: everything that depends on k only
+// (kappa = conj(G) [surface] or i conj(G)/|k|^2 [volume], zero outside the narrow band) is written once per call by the
+// elementwise pre-pass dm_k_kappa, and every warp stages the 32 frequencies it is about to visit from that array into its
+// own 256 bytes of shared memory (one coalesced load per lane, prefetched one chunk ahead).  There is no reduction across
+// threads at all (O(N n_v) backward; :182-186 eq. 13 is the later CSR gather).
 //
 // Shared vertex phases (north_star: "each vertex's phase e^{-ik.v} is computed once per (k-tile, vertex) and reused across
 // its incident triangles").  A patch of 32 triangles has about 28 distinct vertices.  Lane l owns vertex slot l of its
-// patch: per frequency it advances that ONE phase by a
-// complex rotation, multiplies it by kappa and stores A_v = kappa e^{-ik.v} in shared memory; after a __syncwarp the 32
-// triangle lanes read the A_v of their three corners.  Per pair this is 8 FP32 operations + 1 STS + 3 LDS instead of the
-// 24 operations of three private phases.
+// patch: per frequency it advances that ONE phase by a complex rotation, multiplies it by kappa and stores
+// A_v = kappa e^{-ik.v} in shared memory, two frequencies per 16-byte word; after a __syncwarp the 32 triangle lanes read
+// the A_v of their three corners (one LDS.128 per corner and frequency pair).
 //
 // Arithmetic of the generic pair.  With nodes x_j = k.v_j, E_j = e^{-i x_j} and gaps
 // p = x_1-x_0, q = x_2-x_0, r = q-p, eq. 9 is  g = sum_j c_j E_j  with REAL coefficients
 //     c_0 = -1/(pq),  c_1 = 1/(pr),  c_2 = -1/(qr)        (one MUFU.RCP of pqr),
 // and its node derivatives (the closed form of PAPER.md:171-173 eq. 11 with reading R2, regrouped) are
-//     dg/dx_1 = sum_j al_j E_j - i c_1 E_1,   al_0 = q c_0^2, al_2 = -q c_2^2, al_1 = -al_0-al_2   (sum_j c_j = 0)
-//     dg/dx_2 = sum_j be_j E_j - i c_2 E_2,   be_0 = p c_0^2, be_1 = -p c_1^2, be_2 = -be_0-be_1
+//     dg/dx_1 = q (c_0^2 (E_0-E_1) - c_2^2 (E_2-E_1)) - i c_1 E_1
+//     dg/dx_2 = p (c_0^2 (E_0-E_1) + (c_1^2-c_0^2) (E_2-E_1)) - i c_2 E_2
 //     dg/dx_0 = -i g - dg/dx_1 - dg/dx_2.
 // With A_j = kappa E_j the four real numbers a pair contributes are
-//     s0 = Re(kappa g) = sum c_j Re A_j,  sI = Im(kappa g) = sum c_j Im A_j,
-//     sb = Re(kappa dg/dx_1) = sum al_j Re A_j + c_1 Im A_1,   sc likewise,
+//     s0 = Re(kappa g),  sI = Im(kappa g),  sb = Re(kappa dg/dx_1),  sc = Re(kappa dg/dx_2),
 // all taken on differences of the A_j (every coefficient triple sums to zero).
 // Phases advance along z by one complex rotation (rotor e^{-i kstep_z v_z} built in fp64 by the geometry pre-pass) and
-// are re-seeded every SEG (8, 16 or 32) frequencies from exact values: the exact row phase (32-bit integer turns) times a
-// row-independent table of exact z-phases kept in shared memory.
+// are re-seeded every SEG (8, 16 or 32) frequencies from exact values: the exact phase at the start of a "super-segment"
+// of (n_tab+1) SEG frequencies (32-bit integer turns, one accurate sincospi) times a row-independent table of exact
+// z-phases kept in shared memory.  Rows longer than one super-segment are walked super-segment by super-segment, so the
+// kernel has no limit on N_z.
 //
 // Near-degenerate pairs (reading R4).  The derivative coefficients grow like 1/(gap^2 gap'), so a pair
-// with  m1^2 m2 <= tau_b  (m1 <= m2 the two smallest |gaps|)  is excluded from the fast sums (its reciprocal is forced to 0) and flagged in a per-
-// thread bit mask.  After each chunk of <= DM_BF_CHUNK frequencies the WARP pools its flagged pairs in shared memory,
-// sorted by owner, and evaluates them 32 at a time, one pair per lane whatever its owner: the series branch where all
-// gaps are small, the branch-free far-pair variant otherwise.  A segmented warp scan sums the results of one owner and
-// the run's last lane adds them to that owner's shared accumulators -- a fixed order, so the result is bitwise
+// with  m1^2 m2 <= tau_b  (m1 <= m2 the two smallest |gaps|)  is excluded from the fast sums (its reciprocal is forced to
+// 0) and flagged in a per-thread bit mask.  After each chunk of 32 frequencies the flagged pairs are appended, in (owner
+// lane, frequency) order, to a ring buffer the WARP keeps in shared memory ACROSS chunks and rows; whenever the buffer
+// holds 32 pairs the warp evaluates them, one pair per lane whatever its owner (the series branch where all gaps are
+// small, the branch-free far-pair variant otherwise) -- always a full round, the remainder waits for the next chunk.
+// A segmented warp scan sums the results of one (row, owner) run and the run's last lane adds them, weighted with the
+// run's k_x, k_y, to that owner's 13 sums in shared memory, in queue order: a fixed order, so the result is bitwise
 // reproducible (reading R22), and the divergent work is spread evenly over the lanes.
 #pragma once
 #include "dm_kernels.cuh"
@@ -43,14 +46,14 @@
 #ifndef DM_BF_THREADS
 #define DM_BF_THREADS 128
 #endif
+#define DM_BF_WARPS (DM_BF_THREADS / 32)
 #ifndef DM_BF_MINCTA
 #define DM_BF_MINCTA 5         // resident CTAs per SM the register allocation aims at (<= 102 registers)
 #endif
-#define DM_BF_SEG 32            // bits of one flag word
-#define DM_BF_UNR 8             // unroll of the fast loop
-#ifndef DM_BF_STAGE
-#define DM_BF_STAGE 8           // frequencies whose vertex phases are staged in shared memory at a time (divides DM_BF_UNR)
-#endif
+#define DM_BF_CHUNK 32          // frequencies per chunk = one flag word per thread
+#define DM_BF_STAGE 8           // frequencies whose vertex phases are staged in shared memory at a time
+#define DM_BF_NTAB_MAX 8        // seed-table entries per vertex slot: a super-segment is (n_tab + 1) * SEG frequencies
+#define DM_BF_QCAP 256          // ring buffer of flagged pairs per warp (power of two, >= 64)
 #define DM_BF_TREC 4            // float4 per triangle record
 #define DM_BF_VREC 2            // float4 per vertex-slot record
 
@@ -67,12 +70,10 @@ struct DmPatchDev {
 //                              (eb.xyz, longest squared edge)   (ec.xyz, -)   (m_T.xyz, |m_T|)       eb = v_1-v_0, ec = v_2-v_0
 //   vertex    vrec[2i..2i+1] (slot l of the patch):  (u.xyz turns, rho.re)  (rho.im, -, -, -),  rho = e^{-i kstep_z v_z}
 __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int32_t* __restrict__ faces, DmPatchDev pt,
-                                  DmGridDev grid, float4* __restrict__ trec, float4* __restrict__ vrec,
-                                  unsigned int* __restrict__ hmax2_bits)
+                                  DmGridDev grid, float4* __restrict__ trec, float4* __restrict__ vrec)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= pt.n_lanes) return;   // n_lanes is a multiple of the warp size: whole warps leave
-    float h2 = 0.f, e2sum = 0.f;
+    if (i >= pt.n_lanes) return;
     {
         int f = pt.face[i];
         if (f < 0) f = pt.face[i & ~31];   // idle lane: any valid triangle of the patch (lane 0 holds one)
@@ -95,20 +96,15 @@ __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int3
         const float ec[3] = {v[2][0] - v[0][0], v[2][1] - v[0][1], v[2][2] - v[0][2]};
         float m[3];
         dm_cross(eb, ec, m);
-        // edge statistics of the mesh (they scale the flag threshold)
         const float ed[3] = {ec[0] - eb[0], ec[1] - eb[1], ec[2] - eb[2]};
         const float a2 = eb[0] * eb[0] + eb[1] * eb[1] + eb[2] * eb[2], b2 = ec[0] * ec[0] + ec[1] * ec[1] + ec[2] * ec[2],
                     c2 = ed[0] * ed[0] + ed[1] * ed[1] + ed[2] * ed[2];
-        if (pt.face[i] >= 0) {
-            h2 = fmaxf(fmaxf(a2, b2), c2);
-            e2sum = a2 + b2 + c2;
-        }
         const float wf = grid.face_w ? grid.face_w[f] : 1.0f;   // density weight of the face
         const float mn = wf * sqrtf(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
         m[0] *= wf, m[1] *= wf, m[2] *= wf;
         float4* o = trec + (size_t)DM_BF_TREC * i;
         o[0] = make_float4(__uint_as_float(u[0]), __uint_as_float(u[1]), __uint_as_float(u[2]), __uint_as_float(pt.loc[i]));
-        o[1] = make_float4(eb[0], eb[1], eb[2], fmaxf(fmaxf(a2, b2), c2));
+        o[1] = make_float4(eb[0], eb[1], eb[2], fmaxf(fmaxf(a2, b2), c2));   // .w: the triangle's longest squared edge
         o[2] = make_float4(ec[0], ec[1], ec[2], 0.f);
         o[3] = make_float4(m[0], m[1], m[2], mn);
     }
@@ -134,46 +130,59 @@ __global__ void dm_k_bwd_geometry(const float* __restrict__ vertices, const int3
         vrec[DM_BF_VREC * s] = a;
         vrec[DM_BF_VREC * s + 1] = b;
     }
-    dm_edge_stats_add(hmax2_bits, h2, e2sum, grid.edge_fix);
 }
 
-// shared-memory queue of one warp's flagged pairs of one chunk
-#define DM_BF_CHUNK 96          // frequencies per chunk = 3 flag words per thread
-struct DmBfQueue {
-    unsigned char code[32 * DM_BF_CHUNK];  // frequency index inside the chunk, in (owner lane, frequency) order; the
-                                           // owner of entry e is found from the lanes' prefix sums
-};
-
-// what one pair adds to the row sums (plain and k_z-weighted sums of s0, sI, sb, sc)
-struct DmBfRow {
-    float S0, S0z, SI, SIz, SB, SBz, SC, SCz;
-};
+// ---- kappa pre-pass: everything of the backward that depends on the frequency only ------------------------------------
+//   surface: kappa = conj(G);   volume: kappa = i conj(G) / |k|^2  (0 at k = 0: that row is handled by dm_k_corner_grads);
+//   zero outside the narrow band (the cotangent there is ignored).  Same layout as G, slab rows only.
 template <int MODE>
-__device__ __forceinline__ void dm_bf_add(DmBfRow& a, float kz, float om, float s0, float sI, float sb, float sc)
+__global__ void dm_k_kappa(const float2* __restrict__ G, DmGridDev grid, int ix_begin, int ix_end, float2* __restrict__ kappa)
 {
-    if (MODE == 0) {  // volume: omega = k.m_T weights the derivative sums, Q needs k s0
-        sI *= om;
-        sb *= om;
-        sc *= om;
-        a.S0z = fmaf(kz, s0, a.S0z);
+    const long long n_slab = (long long)(ix_end - ix_begin) * grid.ny * grid.nzh;
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= n_slab) return;
+    const int iz = (int)(l % grid.nzh), iy = (int)((l / grid.nzh) % grid.ny);
+    const int ix = ix_begin + (int)(l / ((long long)grid.nzh * grid.ny));
+    const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
+    const size_t o = ((size_t)ix * grid.ny + iy) * grid.nzh + iz;
+    float2 Gk = G[o];
+    if (!dm_in_band(grid, nx, ny, iz)) Gk = make_float2(0.f, 0.f);
+    float2 out;
+    if (MODE == 1) {
+        out = make_float2(Gk.x, -Gk.y);
+    } else {
+        const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny, kz = grid.kstep[2] * iz;
+        const float k2 = kx * kx + ky * ky + kz * kz;
+        const float inv_k2 = (k2 > 0.f) ? 1.0f / k2 : 0.f;
+        out = make_float2(Gk.y * inv_k2, Gk.x * inv_k2);
     }
-    a.S0 += s0;
-    a.SI += sI;
-    a.SIz = fmaf(kz, sI, a.SIz);
-    a.SB += sb;
-    a.SBz = fmaf(kz, sb, a.SBz);
-    a.SC += sc;
-    a.SCz = fmaf(kz, sc, a.SCz);
+    kappa[o] = out;
 }
+
+// shared memory of one warp
+struct DmBfWarp {
+    float4 at4[DM_BF_STAGE / 2][DM_PATCH_MAXV];  // A_v of the patch's vertex slots, two frequencies per word
+    float4 rec[32 * DM_BF_TREC];                 // the patch's triangle records (the pooled path reads other lanes')
+    float wacc[DM_BWD_NSUM][32];                 // the owners' 13 sums of the pooled path
+    uint32_t q[DM_BF_QCAP];                      // ring buffer of flagged pairs: row_local << 17 | owner << 12 | z
+    float2 kbuf[DM_BF_CHUNK];                    // kappa of the chunk's frequencies
+};
+
+// what the pairs of one row add: plain sums and sums weighted with the z index of the frequency
+struct DmBfRow {
+    float S0, T0, SI, TI, SB, TB, SC, TC;
+};
 
 // The fast evaluation of ONE pair (generic closed form) from the staged A_j = kappa e^{-i x_j} of its three corners;
-// returns true when the pair is excluded (flagged) instead.
+// returns true when the pair is excluded (flagged) instead.  zf = z index of the frequency; the gaps are
+// p = prow + zf dpz etc. with dpz = kstep_z eb.z (one rounding more than k_z eb.z, far below the gaps' own error).
 template <int MODE>
-__device__ __forceinline__ bool dm_bf_pair(const float kz, const cf A0, const cf A1, const cf A2, const float prow,
-                                           const float qrow, const float omrow, const float ebz, const float ecz,
-                                           const float mz, const float tau_k, DmBfRow& rs)
+__device__ __forceinline__ bool dm_bf_pair(const float zf, const float A0r, const float A0i, const float A1r, const float A1i,
+                                           const float A2r, const float A2i, const float prow, const float qrow,
+                                           const float omrow, const float dpz, const float dqz, const float dmz,
+                                           const float tau_k, DmBfRow& rs)
 {
-    const float p = fmaf(kz, ebz, prow), q = fmaf(kz, ecz, qrow), r = q - p;
+    const float p = fmaf(zf, dpz, prow), q = fmaf(zf, dqz, qrow), r = q - p;
     const float pqr = (p * q) * r;
     // the largest derivative coefficient is 1/(m1^2 m2), m1 <= m2 <= m3 the sorted |gaps| (m3 = m1 + m2 always): the pair
     // leaves the fast path when m1^2 m2 = m1 |pqr| / m3 <= tau_k  (also catches p = q = r = 0); tau_k = the threshold of
@@ -184,55 +193,153 @@ __device__ __forceinline__ bool dm_bf_pair(const float kz, const cf A0, const cf
     const float R = bad ? 0.f : dm_rcp_approx(pqr);
     const float c0 = -r * R, c1 = q * R, c2 = -p * R;
     const float c0s = c0 * c0, c1s = c1 * c1, c2s = c2 * c2;
-    const float a0 = q * c0s, a2 = -q * c2s;      // al_1 = -al_0 - al_2
-    const float b0 = p * c0s, nb1 = p * c1s;      // be_1 = -nb1, be_2 = -be_0 - be_1
-    const float d01r = A0.re - A1.re, d21r = A2.re - A1.re, d02r = d01r - d21r;
-    const float d01i = A0.im - A1.im, d21i = A2.im - A1.im;
+    const float d01r = A0r - A1r, d21r = A2r - A1r;
+    const float d01i = A0i - A1i, d21i = A2i - A1i;
     const float s0 = fmaf(c0, d01r, c2 * d21r);
-    const float sI = fmaf(c0, d01i, c2 * d21i);
-    const float sb = fmaf(a0, d01r, fmaf(a2, d21r, c1 * A1.im));
-    const float sc = fmaf(b0, d02r, fmaf(nb1, d21r, c2 * A2.im));
-    dm_bf_add<MODE>(rs, kz, fmaf(kz, mz, omrow), s0, sI, sb, sc);
+    float sI = fmaf(c0, d01i, c2 * d21i);
+    const float t0 = c0s * d01r;
+    float sb = fmaf(q, fmaf(-c2s, d21r, t0), c1 * A1i);
+    float sc = fmaf(p, fmaf(c1s - c0s, d21r, t0), c2 * A2i);
+    if (MODE == 0) {  // volume: omega = k.m_T weights the derivative sums, Q needs k s0
+        const float om = fmaf(zf, dmz, omrow);
+        sI *= om;
+        sb *= om;
+        sc *= om;
+        rs.T0 = fmaf(zf, s0, rs.T0);
+    }
+    rs.S0 += s0;
+    rs.SI += sI;
+    rs.TI = fmaf(zf, sI, rs.TI);
+    rs.SB += sb;
+    rs.TB = fmaf(zf, sb, rs.TB);
+    rs.SC += sc;
+    rs.TC = fmaf(zf, sc, rs.TC);
     return bad;
+}
+
+// One round of the pooled slow path: the n (<= 32) oldest queued pairs of the warp, one per lane whatever its owner.
+template <int MODE>
+__device__ __forceinline__ void dm_bf_round(DmBfWarp& W, const int lane, const int n, const int qh, const DmGridDev& grid,
+                                            const int ix_begin, const int row_begin, const float2* __restrict__ kappa)
+{
+    const bool have = lane < n;
+    const uint32_t code = W.q[(qh + lane) & (DM_BF_QCAP - 1)];
+    const int z = (int)(code & 4095u), own = have ? (int)((code >> 12) & 31u) : 0;
+    const int row = row_begin + (have ? (int)(code >> 17) : 0);
+    const int ix = ix_begin + row / grid.ny, iy = row % grid.ny;
+    const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
+    const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny, kz = grid.kstep[2] * z;
+    const float4* orc = W.rec + own * DM_BF_TREC;
+    const float4 q0 = orc[0], q3 = orc[1], q4 = orc[2];
+    const float p = fmaf(kz, q3.z, fmaf(kx, q3.x, ky * q3.y));
+    const float q = fmaf(kz, q4.z, fmaf(kx, q4.x, ky * q4.y));
+    const bool series = fmaxf(fmaxf(fabsf(p), fabsf(q)), fabsf(q - p)) < DM_SERIES_RADIUS;
+    cf psi = {0.f, 0.f}, dp = {0.f, 0.f}, dq = {0.f, 0.f};
+    if (__any_sync(0xffffffffu, have && series)) {
+        cf a, b, c;
+        dm_psi_series<true>(series ? p : 0.f, series ? q : 0.f, a, b, c);
+        if (series) { psi = a; dp = b; dq = c; }
+    }
+    if (__any_sync(0xffffffffu, have && !series)) {
+        cf a, b, c;
+        dm_psi_far_uniform(series ? 0.f : p, series ? 1.f : q, a, b, c);
+        if (!series) { psi = a; dp = b; dq = c; }
+    }
+    const cf E = dm_expmi_turns_fast(dm_phase_turns(nx, ny, z, __float_as_uint(q0.x), __float_as_uint(q0.y),
+                                                    __float_as_uint(q0.z)));
+    float2 kk = make_float2(0.f, 0.f);
+    if (have) kk = kappa[((size_t)ix * grid.ny + iy) * grid.nzh + z];
+    const cf kE = cmul(cf{kk.x, kk.y}, E);
+    const cf kg = cmul(kE, psi);
+    // v[0..3] = s0, sI, sb, sc (the last three weighted with omega in volume mode), v[4..7] = k_z times them
+    float v[8];
+    v[0] = kg.re;
+    v[1] = kg.im;
+    v[2] = kE.re * dp.re - kE.im * dp.im;
+    v[3] = kE.re * dq.re - kE.im * dq.im;
+    if (MODE == 0) {
+        const float4 q5 = orc[3];
+        const float om = fmaf(kz, q5.z, fmaf(kx, q5.x, ky * q5.y));
+        v[1] *= om;
+        v[2] *= om;
+        v[3] *= om;
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) v[4 + i] = kz * v[i];
+    // segmented inclusive scan over the runs of equal (row, owner): head flags from adjacent keys
+    const uint32_t key = have ? (code >> 12) : (0xffffff00u | (uint32_t)lane);
+    const uint32_t kprev = __shfl_up_sync(0xffffffffu, key, 1);
+    const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || kprev != key);
+    const int dist = lane - (31 - __clz((int)(heads & (0xffffffffu >> (31 - lane)))));   // distance to the run's first lane
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (MODE == 1 && i == 4) continue;  // k_z s0 is a volume-mode sum
+            const float x = __shfl_up_sync(0xffffffffu, v[i], o);
+            if (o <= dist) v[i] += x;
+        }
+    }
+    const bool end = have && (lane == 31 || ((heads >> (lane + 1)) & 1u));
+    // two runs of one owner (different rows) can end in the same round: they add in queue order, one rank at a time
+    const uint32_t endmask = __ballot_sync(0xffffffffu, end);
+    int rank = 0;
+    if (end) rank = __popc(__match_any_sync(endmask, own) & ((1u << lane) - 1u));
+    const int maxrank = __reduce_max_sync(0xffffffffu, rank);
+    for (int rk = 0; rk <= maxrank; ++rk) {
+        if (end && rank == rk) {
+            if (MODE == 1) {
+                W.wacc[0][own] += v[0];
+            } else {
+                W.wacc[1][own] = fmaf(kx, v[0], W.wacc[1][own]);
+                W.wacc[2][own] = fmaf(ky, v[0], W.wacc[2][own]);
+                W.wacc[3][own] += v[4];
+            }
+#pragma unroll
+            for (int i = 1; i < 4; ++i) {
+                W.wacc[1 + 3 * i][own] = fmaf(kx, v[i], W.wacc[1 + 3 * i][own]);
+                W.wacc[2 + 3 * i][own] = fmaf(ky, v[i], W.wacc[2 + 3 * i][own]);
+                W.wacc[3 + 3 * i][own] += v[4 + i];
+            }
+        }
+        __syncwarp();
+    }
 }
 
 // ---- A6 backward, fast kernel -----------------------------------------------------------------------------------
 // grid = (n_lanes / DM_BF_THREADS, n_split): one warp per patch; part[(split*13 + s)*n_faces + face] as in
 // dm_k_backward_robust.  BAND = the narrow band is set (band_z holds the in-band z interval of every row).
-// SEG = frequencies between exact phase seeds (8, 16 or 32; chosen by the host so that the seed
-// table fits).  Dynamic shared memory:
-//   2 * nzh float4                      double-buffered rows (kappa.re, kappa.im, k_z, -)
-//   (nseg-1) * 128 float2               seed table ztab[a-1][tid] = e^{-2 pi i (a SEG) u_z} of the thread's vertex
-//                                       slot, a = 1 .. nseg-1, nseg = ceil(nzh/SEG): with the exact row phase
-//                                       e^{-2 pi i (n_x u_x + n_y u_y)} (integer turns, one accurate sincospi per row) a
-//                                       phase is never more than SEG-1 fp32 rotations away from an exact value
-//   4 * DM_BF_STAGE * 32 float2         per warp: A_v = kappa e^{-ik.v} of the patch's vertex slots for DM_BF_STAGE
-//                                       consecutive frequencies
+// SEG = frequencies between exact phase seeds (8, 16 or 32), n_tab <= DM_BF_NTAB_MAX the seed-table entries per vertex
+// slot (a super-segment is (n_tab + 1) SEG frequencies); both chosen by the host.  rows_per_split <= 32768.
+// Dynamic shared memory: n_tab * DM_BF_THREADS float2, ztab[a][tid] = e^{-2 pi i ((a+1) SEG) u_z} of the thread's vertex
+// slot: with the exact super-segment phase a phase is never more than SEG-1 fp32 rotations away from an exact value.
 template <int MODE, int SEG, bool BAND>
 __global__ void __launch_bounds__(DM_BF_THREADS, DM_BF_MINCTA)
 dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__ vrec_g, DmPatchDev pt, int n_faces,
-                   DmGridDev grid, int ix_begin, int ix_end, int rows_per_split, float tau_b,
-                   const float2* __restrict__ G, const int2* __restrict__ band_z, float* __restrict__ part)
+                   DmGridDev grid, int ix_begin, int ix_end, int rows_per_split, float tau_b, int n_tab,
+                   const float2* __restrict__ kappa, const int2* __restrict__ band_z, float* __restrict__ part)
 {
-    static_assert(SEG == 8 || SEG == 16 || SEG == 32, "SEG divides the 32-bit flag word");
-    static_assert(DM_BF_UNR % DM_BF_STAGE == 0 && SEG % DM_BF_UNR == 0, "stages tile the unrolled body, bodies tile a segment");
-    extern __shared__ float4 dm_bf_smem[];
-    __shared__ DmBfQueue queue[DM_BF_THREADS / 32];
-    __shared__ float4 trec[DM_BF_THREADS * DM_BF_TREC];    // this CTA's triangle records (the pooled path reads other lanes')
-    __shared__ float wacc[(DM_BF_THREADS / 32) * 8 * 32];  // per warp: 8 row sums x 32 owners, filled by the pooled path
-    float4* const sk = dm_bf_smem;
+    static_assert(SEG == 8 || SEG == 16 || SEG == 32, "SEG is a multiple of the stage and divides the chunk");
+    extern __shared__ float2 dm_bf_ztab[];
+    __shared__ DmBfWarp wsm[DM_BF_WARPS];
     const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+    DmBfWarp& W = wsm[wrp];
     const int gl = blockIdx.x * DM_BF_THREADS + tid;       // global lane = 32 * patch + lane
     const int face = pt.face[gl];
     const bool live = face >= 0;
-    const float4 r0 = trec_g[(size_t)DM_BF_TREC * gl], r3 = trec_g[(size_t)DM_BF_TREC * gl + 1],
-                 r4 = trec_g[(size_t)DM_BF_TREC * gl + 2], r5 = trec_g[(size_t)DM_BF_TREC * gl + 3];
-    trec[tid * DM_BF_TREC + 0] = r0;
-    trec[tid * DM_BF_TREC + 1] = r3;
-    trec[tid * DM_BF_TREC + 2] = r4;
-    trec[tid * DM_BF_TREC + 3] = r5;
-    const uint32_t loc = __float_as_uint(r0.w);
-    const int l0 = (int)(loc & 255u), l1 = (int)((loc >> 8) & 255u), l2 = (int)((loc >> 16) & 255u);
+    float dpz, dqz, dmz;
+    int l0, l1, l2;
+    {
+        const float4 r0 = trec_g[(size_t)DM_BF_TREC * gl], r1 = trec_g[(size_t)DM_BF_TREC * gl + 1],
+                     r2 = trec_g[(size_t)DM_BF_TREC * gl + 2], r3 = trec_g[(size_t)DM_BF_TREC * gl + 3];
+        W.rec[lane * DM_BF_TREC + 0] = r0;
+        W.rec[lane * DM_BF_TREC + 1] = r1;
+        W.rec[lane * DM_BF_TREC + 2] = r2;
+        W.rec[lane * DM_BF_TREC + 3] = r3;
+        const uint32_t loc = __float_as_uint(r0.w);
+        l0 = (int)(loc & 255u), l1 = (int)((loc >> 8) & 255u), l2 = (int)((loc >> 16) & 255u);
+        dpz = grid.kstep[2] * r1.z, dqz = grid.kstep[2] * r2.z, dmz = grid.kstep[2] * r3.z;
+    }
     // the vertex slot this lane owns (slot lane of its patch)
     const float4 va0 = vrec_g[(size_t)DM_BF_VREC * gl], va1 = vrec_g[(size_t)DM_BF_VREC * gl + 1];
     const uint32_t uax = __float_as_uint(va0.x), uay = __float_as_uint(va0.y), uaz = __float_as_uint(va0.z);
@@ -241,286 +348,194 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
     const int n_rows = (ix_end - ix_begin) * grid.ny;
     const int row_begin = blockIdx.y * rows_per_split;
     const int row_end = min(n_rows, row_begin + rows_per_split);
-    DmBfQueue& Q = queue[wrp];
-    const float4* const wrec = trec + wrp * 32 * DM_BF_TREC;   // records of this warp's 32 triangles
+    const int SS = (n_tab + 1) * SEG;                      // frequencies per super-segment
 
-    // seed table (row-independent): exact z-phases of this thread's vertex slots at every multiple of SEG
-    const int nseg = (nzh + SEG - 1) / SEG;
-    float2* const ztab = reinterpret_cast<float2*>(dm_bf_smem + 2 * nzh);
-    float2* const at = ztab + (size_t)(nseg - 1) * DM_BF_THREADS + wrp * DM_BF_STAGE * DM_PATCH_MAXV;
-    for (int a = 1; a < nseg; ++a) {
-        const uint32_t za = (uint32_t)(a * SEG);
-        const cf z0 = dm_expmi_turns(za * uaz);
-        ztab[(a - 1) * DM_BF_THREADS + tid] = make_float2(z0.re, z0.im);
+    // seed table (row-independent): exact z-phases of this thread's vertex slot at the multiples of SEG
+    for (int a = 0; a < n_tab; ++a) {
+        const cf z0 = dm_expmi_turns((uint32_t)((a + 1) * SEG) * uaz);
+        dm_bf_ztab[a * DM_BF_THREADS + tid] = make_float2(z0.re, z0.im);
     }
-
 #pragma unroll
-    for (int i = 0; i < 8; ++i) wacc[i * DM_BF_THREADS + tid] = 0.f;
+    for (int s = 0; s < DM_BWD_NSUM; ++s) W.wacc[s][lane] = 0.f;
+    __syncwarp();
+
     // acc: [0] S0 | [1..3] Q | [4..6] W | [7..9] Vb | [10..12] Vc   (dm_k_backward_robust)
     float acc[DM_BWD_NSUM];
 #pragma unroll
     for (int s = 0; s < DM_BWD_NSUM; ++s) acc[s] = 0.f;
+    int qh = 0, qlen = 0;                                  // ring buffer of flagged pairs (warp-uniform)
 
-    // stage kappa and k_z of one row into buffer b
-    auto stage_row = [&](int row, int b) {
-        const int ix = ix_begin + row / grid.ny, iy = row % grid.ny;
-        const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
-        const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
-        const float2* Grow = G + ((size_t)ix * grid.ny + iy) * nzh;
-        for (int iz = tid; iz < nzh; iz += DM_BF_THREADS) {
-            const float kz = grid.kstep[2] * iz;
-            float2 Gk = Grow[iz];
-            if (BAND && !dm_in_band(grid, nx, ny, iz)) Gk = make_float2(0.f, 0.f);  // narrow band: the cotangent outside is ignored
-            float4 o;
-            if (MODE == 1) {
-                o = make_float4(Gk.x, -Gk.y, kz, 0.f);                       // conj(G)
-            } else {
-                const float k2 = kx * kx + ky * ky + kz * kz;
-                const float inv_k2 = (k2 > 0.f) ? 1.0f / k2 : 0.f;           // k = 0 is handled by dm_k_corner_grads
-                o = make_float4(Gk.y * inv_k2, Gk.x * inv_k2, kz, 0.f);      // i conj(G) / |k|^2
-            }
-            sk[b * nzh + iz] = o;
-        }
-    };
-
-    // one stage of n <= DM_BF_STAGE frequencies starting at z: every lane writes A_v of its vertex slot(s), then every
-    // lane evaluates its triangle at those frequencies; returns the flags of the stage (bit j = frequency z + j)
-    auto run_stage = [&](const float4* skr, int z, int n, bool full, cf& Ea, float prow, float qrow, float omrow,
-                         float tau_row, DmBfRow& rs) -> uint32_t {
-        if (full) {
-#pragma unroll
-            for (int j = 0; j < DM_BF_STAGE; ++j) {
-                const float4 kk = skr[z + j];
-                const cf A = cmul(cf{kk.x, kk.y}, Ea);
-                at[j * DM_PATCH_MAXV + lane] = make_float2(A.re, A.im);
-                Ea = cmul(Ea, rhoa);
-            }
-        } else {
-#pragma unroll 1
-            for (int j = 0; j < n; ++j) {
-                const float4 kk = skr[z + j];
-                const cf A = cmul(cf{kk.x, kk.y}, Ea);
-                at[j * DM_PATCH_MAXV + lane] = make_float2(A.re, A.im);
-                Ea = cmul(Ea, rhoa);
-            }
-        }
-        __syncwarp();
-        uint32_t sf = 0;
-        if (full) {
-#pragma unroll
-            for (int j = 0; j < DM_BF_STAGE; ++j) {
-                const float kz = skr[z + j].z;
-                const float2 a0 = at[j * DM_PATCH_MAXV + l0], a1 = at[j * DM_PATCH_MAXV + l1], a2 = at[j * DM_PATCH_MAXV + l2];
-                if (dm_bf_pair<MODE>(kz, cf{a0.x, a0.y}, cf{a1.x, a1.y}, cf{a2.x, a2.y}, prow, qrow, omrow, r3.z, r4.z, r5.z,
-                                     tau_row, rs))
-                    sf |= 1u << j;
-            }
-        } else {
-#pragma unroll 1
-            for (int j = 0; j < n; ++j) {
-                const float kz = skr[z + j].z;
-                const float2 a0 = at[j * DM_PATCH_MAXV + l0], a1 = at[j * DM_PATCH_MAXV + l1], a2 = at[j * DM_PATCH_MAXV + l2];
-                if (dm_bf_pair<MODE>(kz, cf{a0.x, a0.y}, cf{a1.x, a1.y}, cf{a2.x, a2.y}, prow, qrow, omrow, r3.z, r4.z, r5.z,
-                                     tau_row, rs))
-                    sf |= 1u << j;
-            }
-        }
-        __syncwarp();
-        return sf;
-    };
-
-    if (row_begin < row_end) stage_row(row_begin, 0);
-    __syncthreads();
-    for (int row = row_begin; row < row_end; ++row) {
-        const int b = (row - row_begin) & 1;
-        if (row + 1 < row_end) stage_row(row + 1, b ^ 1);
-        const float4* __restrict__ skr = sk + b * nzh;
-        const int ix = ix_begin + row / grid.ny, iy = row % grid.ny;
-        const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
-        const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
-        const float prow = fmaf(kx, r3.x, ky * r3.y), qrow = fmaf(kx, r4.x, ky * r4.y);
-        const float omrow = fmaf(kx, r5.x, ky * r5.y);
-        // flag threshold of this triangle on this row: tau_b max(1, (|k| h_T / 12)^3), |k| the largest of the row, h_T the
-        // longest edge of the triangle.  On a triangle that is large for the grid (|k| h >> 1) the rounding error of a gap
-        // k.e grows like |k| h while the integral decays like 1/(|k| h)^2; the factor is exactly 1 when |k| h_T <= 12
-        const float kzm = grid.kstep[2] * (float)(nzh - 1);
-        const float kh2 = (1.0f / 144.0f) * (kx * kx + ky * ky + kzm * kzm) * trec[tid * DM_BF_TREC + 1].w;   // (re-read: one register less)
-        const float tau_row = tau_b * fmaxf(1.0f, kh2 * sqrtf(kh2));
-        // exact row phase e^{-i (k_x v_x + k_y v_y)} of the lane's vertex slot
-        const cf Xa = dm_expmi_turns((uint32_t)nx * uax + (uint32_t)ny * uay);
-        DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-
-        // narrow band: only the in-band interval of the row, started at a seed position
-        int z_lo = 0, z_hi = nzh;
+    // in-band z interval of a row, started at a seed position (the whole row without a band)
+    auto row_range = [&](int row, int& lo, int& hi) {
+        lo = 0, hi = nzh;
         if (BAND) {
-            const int2 bz = band_z[ix * grid.ny + iy];
-            z_lo = bz.x & ~(SEG - 1);
-            z_hi = bz.y;
+            const int2 bz = band_z[ix_begin * grid.ny + row];
+            lo = bz.x & ~(SEG - 1);
+            hi = bz.y;
         }
-        for (int zc = z_lo; zc < z_hi; zc += DM_BF_CHUNK) {
-            const int clen = min(DM_BF_CHUNK, z_hi - zc);
-            uint32_t fl[DM_BF_CHUNK / 32];
-            // ---- fast pass over the chunk: bodies of DM_BF_UNR frequencies, exact seeds every SEG ---------------------
-            cf Ea = Xa;
-#pragma unroll
-            for (int w = 0; w < DM_BF_CHUNK / 32; ++w) {
-                uint32_t word = 0;
-                const int wbeg = zc + 32 * w;
-                const int wlen = min(32, zc + clen - wbeg);
-                if (wlen > 0) {
-                    const int nfull = wlen / DM_BF_UNR;
-                    int z0 = wbeg;
-#pragma unroll 1
-                    for (int s = 0; s <= nfull; ++s, z0 += DM_BF_UNR) {
-                        const int len = (s < nfull) ? DM_BF_UNR : wlen - nfull * DM_BF_UNR;
-                        if (len == 0) break;
-                        if ((z0 & (SEG - 1)) == 0) {   // exact seed
-                            Ea = Xa;
-                            if (z0 > 0) {
-                                const float2 a0 = ztab[(size_t)(z0 / SEG - 1) * DM_BF_THREADS + tid];
-                                Ea = cmul(Xa, cf{a0.x, a0.y});
-                            }
-                        }
-                        uint32_t sf = 0;
-                        if (len == DM_BF_UNR) {
-#pragma unroll
-                            for (int h = 0; h < DM_BF_UNR / DM_BF_STAGE; ++h)
-                                sf |= run_stage(skr, z0 + h * DM_BF_STAGE, DM_BF_STAGE, true, Ea, prow, qrow, omrow, tau_row, rs)
-                                      << (h * DM_BF_STAGE);
-                        } else {
-#pragma unroll 1
-                            for (int j0 = 0; j0 < len; j0 += DM_BF_STAGE)
-                                sf |= run_stage(skr, z0 + j0, min(DM_BF_STAGE, len - j0), false, Ea, prow, qrow, omrow, tau_row, rs) << j0;
-                        }
-                        word |= sf << (s * DM_BF_UNR);
-                    }
+    };
+    const float2* krow = kappa + ((size_t)ix_begin * grid.ny + row_begin) * nzh;
+    float2 knext = make_float2(0.f, 0.f);                  // kappa of this lane's frequency of the NEXT chunk
+    int pref_row = -1;                                     // row whose first chunk knext holds
+    int ix = ix_begin + row_begin / grid.ny, iy = row_begin % grid.ny;
+
+    for (int row = row_begin; row < row_end; ++row, krow += nzh) {
+        int z_lo, z_hi;
+        row_range(row, z_lo, z_hi);
+        int zn_lo = 0, zn_hi = 0;                          // the next row's interval (for the prefetch)
+        if (row + 1 < row_end) row_range(row + 1, zn_lo, zn_hi);
+        const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
+        if (++iy == grid.ny) iy = 0, ++ix;
+        if (z_lo >= z_hi) continue;
+        const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
+        float prow, qrow, omrow, tau_row;
+        {
+            const float4 r1 = W.rec[lane * DM_BF_TREC + 1], r2 = W.rec[lane * DM_BF_TREC + 2], r3 = W.rec[lane * DM_BF_TREC + 3];
+            prow = fmaf(kx, r1.x, ky * r1.y), qrow = fmaf(kx, r2.x, ky * r2.y), omrow = fmaf(kx, r3.x, ky * r3.y);
+            // flag threshold of this triangle on this row: tau_b max(1, (|k| h_T / 12)^3), |k| the largest of the row, h_T
+            // the longest edge of the triangle.  On a triangle that is large for the grid (|k| h >> 1) the rounding error of
+            // a gap k.e grows like |k| h while the integral decays like 1/(|k| h)^2; the factor is 1 when |k| h_T <= 12
+            const float kzm = grid.kstep[2] * (float)(nzh - 1);
+            const float kh2 = (1.0f / 144.0f) * (kx * kx + ky * ky + kzm * kzm) * r1.w;
+            tau_row = tau_b * fmaxf(1.0f, kh2 * sqrtf(kh2));
+        }
+        const uint32_t xturns = (uint32_t)nx * uax + (uint32_t)ny * uay;   // exact row phase of the lane's vertex slot
+        if (pref_row != row) knext = (z_lo + lane < z_hi) ? krow[z_lo + lane] : make_float2(0.f, 0.f);
+        DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        cf Xs = {1.f, 0.f}, Ea = {1.f, 0.f};
+        int zs = z_lo;
+        for (int z = z_lo; z < z_hi;) {
+            if (z == zs) Xs = dm_expmi_turns(xturns + (uint32_t)zs * uaz);   // exact phase at the super-segment start
+            const int ze = min(zs + SS, z_hi);
+            const int clen = min(DM_BF_CHUNK, ze - z);
+            // ---- stage kappa of the chunk, prefetch the next chunk's ------------------------------------------------
+            W.kbuf[lane] = knext;
+            __syncwarp();
+            {
+                const int zn = z + clen;
+                if (zn < z_hi) {          // (entries past the next chunk's end are loaded but never read)
+                    knext = (zn + lane < z_hi) ? krow[zn + lane] : make_float2(0.f, 0.f);
+                } else if (zn_lo < zn_hi) {
+                    knext = (zn_lo + lane < zn_hi) ? krow[nzh + zn_lo + lane] : make_float2(0.f, 0.f);
+                    pref_row = row + 1;
                 }
-                fl[w] = live ? word : 0u;
             }
-            // ---- pooled slow path -------------------------------------------------------------------------------------
-            int cnt = 0;
-#pragma unroll
-            for (int sg = 0; sg < DM_BF_CHUNK / DM_BF_SEG; ++sg) cnt += __popc(fl[sg]);
-            if (__any_sync(0xffffffffu, cnt != 0)) {
-                int off = cnt;  // inclusive prefix sum over lanes
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int n = __shfl_up_sync(0xffffffffu, off, o);
-                    if (lane >= o) off += n;
-                }
-                const int total = __shfl_sync(0xffffffffu, off, 31);
-                // owners queue their pairs in (lane, frequency) order
-                int w = off - cnt;
-#pragma unroll
-                for (int sg = 0; sg < DM_BF_CHUNK / DM_BF_SEG; ++sg) {
-                    uint32_t f = fl[sg];
-                    while (f) {
-                        const int j = __ffs(f) - 1;
-                        f &= f - 1;
-                        Q.code[w++] = (unsigned char)(sg * DM_BF_SEG + j);
+            // ---- fast pass over the chunk: bodies of DM_BF_STAGE frequencies, exact seeds every SEG -----------------
+            uint32_t word = 0;
+            int zloc = 0;
+#pragma unroll 1
+            for (; zloc < clen; zloc += DM_BF_STAGE) {
+                const int z0 = z + zloc;
+                if (((z0 - zs) & (SEG - 1)) == 0) {   // exact seed
+                    Ea = Xs;
+                    if (z0 > zs) {
+                        const float2 a0 = dm_bf_ztab[((z0 - zs) / SEG - 1) * DM_BF_THREADS + tid];
+                        Ea = cmul(Xs, cf{a0.x, a0.y});
                     }
                 }
-                __syncwarp();
-                // rounds of 32 queued pairs: every lane evaluates one pair; a segmented scan over the (sorted) owners sums
-                // the pairs of one owner, and the last lane of each run adds the run into the owner's shared accumulators
-                for (int base = 0; base < total; base += 32) {
-                    const int e = base + lane;
-                    const bool have = e < total;
-                    // owner of entry e = number of lanes whose inclusive prefix sum is <= e (binary search by shuffles)
-                    int own = 0;
+                const float zf = (float)z0;
+                uint32_t sf = 0;
+                if (zloc + DM_BF_STAGE <= clen) {
+                    // every lane writes A_v of its vertex slot for 8 frequencies, then evaluates its triangle at them
+                    const float4* kb4 = reinterpret_cast<const float4*>(W.kbuf) + (zloc >> 1);
 #pragma unroll
-                    for (int st = 16; st > 0; st >>= 1) {
-                        const int v = __shfl_sync(0xffffffffu, off, own + st - 1);
-                        if (v <= e) own += st;
-                    }
-                    own = have ? own : 0;
-                    const int ol = have ? own : -1 - lane, jz = zc + (have ? (int)Q.code[e] : 0);
-                    const float4* orc = wrec + own * 4;
-                    const float4 q0 = orc[0], q3 = orc[1], q4 = orc[2], q5 = orc[3];
-                    const float4 kk = skr[jz];
-                    const float kz = kk.z;
-                    const float p = fmaf(kz, q3.z, fmaf(kx, q3.x, ky * q3.y));
-                    const float q = fmaf(kz, q4.z, fmaf(kx, q4.x, ky * q4.y));
-                    const bool series = fmaxf(fmaxf(fabsf(p), fabsf(q)), fabsf(q - p)) < DM_SERIES_RADIUS;
-                    cf psi = {0.f, 0.f}, dp = {0.f, 0.f}, dq = {0.f, 0.f};
-                    if (__any_sync(0xffffffffu, have && series)) {
-                        cf a, b, c;
-                        dm_psi_series<true>(series ? p : 0.f, series ? q : 0.f, a, b, c);
-                        if (series) { psi = a; dp = b; dq = c; }
-                    }
-                    if (__any_sync(0xffffffffu, have && !series)) {
-                        cf a, b, c;
-                        dm_psi_far_uniform(series ? 0.f : p, series ? 1.f : q, a, b, c);
-                        if (!series) { psi = a; dp = b; dq = c; }
-                    }
-                    const cf E = dm_expmi_turns_fast(dm_phase_turns(nx, ny, jz, __float_as_uint(q0.x), __float_as_uint(q0.y),
-                                                                    __float_as_uint(q0.z)));
-                    const cf kE = cmul(cf{kk.x, kk.y}, E);
-                    const cf kg = cmul(kE, psi);
-                    DmBfRow v = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-                    if (have)
-                        dm_bf_add<MODE>(v, kz, fmaf(kz, q5.z, fmaf(kx, q5.x, ky * q5.y)), kg.re, kg.im,
-                                        kE.re * dp.re - kE.im * dp.im, kE.re * dq.re - kE.im * dq.im);
-                    float vv[8] = {v.S0, v.S0z, v.SI, v.SIz, v.SB, v.SBz, v.SC, v.SCz};
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int ko = __shfl_up_sync(0xffffffffu, ol, o);
-                        const bool take = lane >= o && ko == ol;
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            if (MODE == 1 && i == 1) continue;  // S0z is a volume-mode sum
-                            const float x = __shfl_up_sync(0xffffffffu, vv[i], o);
-                            if (take) vv[i] += x;
-                        }
-                    }
-                    const int kn = __shfl_down_sync(0xffffffffu, ol, 1);
-                    if (have && (lane == 31 || kn != ol)) {
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            if (MODE == 1 && i == 1) continue;
-                            wacc[(wrp * 8 + i) * 32 + ol] += vv[i];
-                        }
+                    for (int jp = 0; jp < DM_BF_STAGE / 2; ++jp) {
+                        const float4 k4 = kb4[jp];
+                        const cf A = cmul(cf{k4.x, k4.y}, Ea);
+                        Ea = cmul(Ea, rhoa);
+                        const cf B = cmul(cf{k4.z, k4.w}, Ea);
+                        Ea = cmul(Ea, rhoa);
+                        W.at4[jp][lane] = make_float4(A.re, A.im, B.re, B.im);
                     }
                     __syncwarp();
-                }
-                // owners take their sums back (and clear them)
-                if (cnt != 0) {
-                    float* a = wacc + wrp * 8 * 32 + lane;
-                    rs.S0 += a[0];
-                    if (MODE == 0) rs.S0z += a[32];
-                    rs.SI += a[64];
-                    rs.SIz += a[96];
-                    rs.SB += a[128];
-                    rs.SBz += a[160];
-                    rs.SC += a[192];
-                    rs.SCz += a[224];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) a[32 * i] = 0.f;
+                    for (int jp = 0; jp < DM_BF_STAGE / 2; ++jp) {
+                        const float4 a0 = W.at4[jp][l0], a1 = W.at4[jp][l1], a2 = W.at4[jp][l2];
+                        if (dm_bf_pair<MODE>(zf + (float)(2 * jp), a0.x, a0.y, a1.x, a1.y, a2.x, a2.y, prow, qrow, omrow, dpz, dqz,
+                                             dmz, tau_row, rs))
+                            sf |= 1u << (2 * jp);
+                        if (dm_bf_pair<MODE>(zf + (float)(2 * jp + 1), a0.z, a0.w, a1.z, a1.w, a2.z, a2.w, prow, qrow, omrow, dpz,
+                                             dqz, dmz, tau_row, rs))
+                            sf |= 1u << (2 * jp + 1);
+                    }
+                    __syncwarp();
+                } else {
+                    // ragged end of the chunk: one frequency at a time
+#pragma unroll 1
+                    for (int j = 0; zloc + j < clen; ++j) {
+                        const float2 k1 = W.kbuf[zloc + j];
+                        const cf A = cmul(cf{k1.x, k1.y}, Ea);
+                        Ea = cmul(Ea, rhoa);
+                        W.at4[0][lane] = make_float4(A.re, A.im, 0.f, 0.f);
+                        __syncwarp();
+                        const float4 a0 = W.at4[0][l0], a1 = W.at4[0][l1], a2 = W.at4[0][l2];
+                        if (dm_bf_pair<MODE>(zf + (float)j, a0.x, a0.y, a1.x, a1.y, a2.x, a2.y, prow, qrow, omrow, dpz, dqz, dmz,
+                                             tau_row, rs))
+                            sf |= 1u << j;
+                        __syncwarp();
+                    }
                 }
-                __syncwarp();
+                word |= sf << zloc;
             }
+            word = live ? word : 0u;
+            // ---- queue the flagged pairs of the chunk in (lane, frequency) order; evaluate whole rounds of 32 ---------
+            int cnt = __popc(word);
+            if (__any_sync(0xffffffffu, cnt != 0)) {
+                const uint32_t base = ((uint32_t)(row - row_begin) << 17) | ((uint32_t)lane << 12) | (uint32_t)z;
+                for (;;) {
+                    int off = cnt;  // inclusive prefix sum over lanes
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int n = __shfl_up_sync(0xffffffffu, off, o);
+                        if (lane >= o) off += n;
+                    }
+                    const int total = __shfl_sync(0xffffffffu, off, 31);
+                    const int room = DM_BF_QCAP - qlen;
+                    int pos = off - cnt;
+                    while (word != 0u && pos < room) {
+                        const int j = __ffs(word) - 1;
+                        word &= word - 1;
+                        W.q[(qh + qlen + pos) & (DM_BF_QCAP - 1)] = base + (uint32_t)j;
+                        ++pos;
+                    }
+                    qlen += min(total, room);
+                    __syncwarp();
+                    while (qlen >= 32) {
+                        dm_bf_round<MODE>(W, lane, 32, qh, grid, ix_begin, row_begin, kappa);
+                        qh = (qh + 32) & (DM_BF_QCAP - 1);
+                        qlen -= 32;
+                    }
+                    if (total <= room) break;
+                    cnt = __popc(word);
+                }
+            }
+            z += clen;
+            if (z == ze) zs = ze;
         }
-        // fold the row into the 13 sums
+        // fold the row into the 13 sums (the z-weighted sums carry the z index: k_z = kstep_z z)
         if (MODE == 1) {
             acc[0] += rs.S0;
         } else {
             acc[1] = fmaf(kx, rs.S0, acc[1]);
             acc[2] = fmaf(ky, rs.S0, acc[2]);
-            acc[3] += rs.S0z;
+            acc[3] = fmaf(grid.kstep[2], rs.T0, acc[3]);
         }
         acc[4] = fmaf(kx, rs.SI, acc[4]);
         acc[5] = fmaf(ky, rs.SI, acc[5]);
-        acc[6] += rs.SIz;
+        acc[6] = fmaf(grid.kstep[2], rs.TI, acc[6]);
         acc[7] = fmaf(kx, rs.SB, acc[7]);
         acc[8] = fmaf(ky, rs.SB, acc[8]);
-        acc[9] += rs.SBz;
+        acc[9] = fmaf(grid.kstep[2], rs.TB, acc[9]);
         acc[10] = fmaf(kx, rs.SC, acc[10]);
         acc[11] = fmaf(ky, rs.SC, acc[11]);
-        acc[12] += rs.SCz;
-        __syncthreads();  // next row's buffer is complete; this row's buffer may be overwritten
+        acc[12] = fmaf(grid.kstep[2], rs.TC, acc[12]);
     }
+    // the pairs still queued (< 32), then the pooled path's sums
+    if (qlen > 0) dm_bf_round<MODE>(W, lane, qlen, qh, grid, ix_begin, row_begin, kappa);
+    __syncwarp();
     if (live) {
 #pragma unroll
-        for (int s = 0; s < DM_BWD_NSUM; ++s) part[((size_t)blockIdx.y * DM_BWD_NSUM + s) * n_faces + face] = acc[s];
+        for (int s = 0; s < DM_BWD_NSUM; ++s)
+            part[((size_t)blockIdx.y * DM_BWD_NSUM + s) * n_faces + face] = acc[s] + W.wacc[s][lane];
     }
 }
