@@ -266,7 +266,6 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     // a row longer than (n_tab + 1) seg frequencies is walked in several super-segments
     const int seg = nzh <= 72 ? 8 : (nzh <= 144 ? 16 : 32);
     const int n_tab = std::min(DM_BF_NTAB_MAX, (nzh + seg - 1) / seg - 1);
-    const size_t tab_smem = (size_t)n_tab * DM_BF_THREADS * sizeof(float2);
     int rc;
     const bool robust = p->bwd_path != 0 || p->weights_robust || rps > 32768;
     p->last_bwd_path = robust ? 1 : 0;
@@ -284,7 +283,7 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
             dm_k_kappa<0><<<(unsigned)((n_slab + 255) / 256), 256, 0, p->stream>>>((const float2*)G_dev, p->gd, p->ix_begin, p->ix_end, p->kappa);
         if ((rc = check_launch(p))) return rc;
 #define DM_LAUNCH_BF2(MODE, SEG, BAND)                                                                                   \
-    dm_k_backward_fast<MODE, SEG, BAND><<<grid, DM_BF_THREADS, tab_smem, p->stream>>>(                                   \
+    dm_k_backward_fast<MODE, SEG, BAND><<<grid, DM_BF_THREADS, 0, p->stream>>>(                                   \
         p->btrec, p->bvrec, pt, p->n_faces, p->gd, p->ix_begin, p->ix_end, rps, tau_b_eff, n_tab, p->kappa, p->band_z, p->part)
 #define DM_LAUNCH_BF(MODE, SEG)                                                                                          \
     do {                                                                                                                 \
@@ -477,7 +476,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
         // k-splits of the backward: a small mesh has few triangle blocks, so it needs many splits to fill the machine
         // (up to 48 CTAs per SM slot), within 64 M floats of partial sums
         {
-            const long long tri_blocks = ((long long)n_faces + DM_BF_THREADS - 1) / DM_BF_THREADS;
+            const long long tri_blocks = ((long long)n_faces + 127) / 128;
             long long m = ((long long)p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
             m = std::min<long long>(m, (64LL << 20) / ((long long)DM_BWD_NSUM * n_faces));
             p->n_split_max = (int)std::max<long long>(64, std::min<long long>(m, 4096));

@@ -43,17 +43,15 @@
 #include "dm_kernels.cuh"
 #include "dm_patches.h"
 
-#ifndef DM_BF_THREADS
-#define DM_BF_THREADS 128
-#endif
-#define DM_BF_WARPS (DM_BF_THREADS / 32)
+#define DM_BF_THREADS 32        // one warp = one patch per CTA: the warps share nothing, and a one-warp CTA addresses its
+                                // shared memory with constants
 #ifndef DM_BF_MINCTA
-#define DM_BF_MINCTA 5         // resident CTAs per SM the register allocation aims at (<= 102 registers)
+#define DM_BF_MINCTA 20        // resident CTAs (= warps) per SM the register allocation aims at (<= 102 registers)
 #endif
 #define DM_BF_CHUNK 32          // frequencies per chunk = one flag word per thread
 #define DM_BF_STAGE 8           // frequencies whose vertex phases are staged in shared memory at a time
 #define DM_BF_NTAB_MAX 8        // seed-table entries per vertex slot: a super-segment is (n_tab + 1) * SEG frequencies
-#define DM_BF_QCAP 256          // ring buffer of flagged pairs per warp (power of two, >= 64)
+#define DM_BF_QCAP 64           // ring buffer of flag words per warp: < 32 carried over + <= 32 new per chunk
 #define DM_BF_TREC 4            // float4 per triangle record
 #define DM_BF_VREC 2            // float4 per vertex-slot record
 
@@ -159,13 +157,15 @@ __global__ void dm_k_kappa(const float2* __restrict__ G, DmGridDev grid, int ix_
     kappa[o] = out;
 }
 
-// shared memory of one warp
+// shared memory of one warp = one CTA (static, so every access is base + constant offset)
 struct DmBfWarp {
     float4 at4[DM_BF_STAGE / 2][DM_PATCH_MAXV];  // A_v of the patch's vertex slots, two frequencies per word
     float4 rec[32 * DM_BF_TREC];                 // the patch's triangle records (the pooled path reads other lanes')
-    float wacc[DM_BWD_NSUM][32];                 // the owners' 13 sums of the pooled path
-    uint32_t q[DM_BF_QCAP];                      // ring buffer of flagged pairs: row_local << 17 | owner << 12 | z
+    uint4 wq[DM_BF_QCAP];                        // ring buffer of flag words: (row_local << 17 | owner << 12 | z of bit 0,
+                                                 //   flag word, n_x & 0xffff | n_y << 16, -)
+    float2 ztab[DM_BF_NTAB_MAX][32];             // seed table: e^{-2 pi i ((a+1) SEG) u_z} of the lanes' vertex slots
     float2 kbuf[DM_BF_CHUNK];                    // kappa of the chunk's frequencies
+    int src[32];                                 // pooled path: the lane that holds the sums of owner l this round
 };
 
 // what the pairs of one row add: plain sums and sums weighted with the z index of the frequency
@@ -173,14 +173,16 @@ struct DmBfRow {
     float S0, T0, SI, TI, SB, TB, SC, TC;
 };
 
-// The fast evaluation of ONE pair (generic closed form) from the staged A_j = kappa e^{-i x_j} of its three corners;
-// returns true when the pair is excluded (flagged) instead.  zf = z index of the frequency; the gaps are
-// p = prow + zf dpz etc. with dpz = kstep_z eb.z (one rounding more than k_z eb.z, far below the gaps' own error).
+// The fast evaluation of ONE pair (generic closed form) from the staged A_j = kappa e^{-i x_j} of its three corners.
+// An excluded (flagged) pair sets `bit` in `flags` instead and accumulates nothing: the seven accumulations and the flag
+// are ONE predicated PTX block (the compiler would otherwise merge the two outcomes with a select per sum).
+// zf = z index of the frequency; the gaps are p = prow + zf dpz etc. with dpz = kstep_z eb.z (one rounding more than
+// k_z eb.z, far below the gaps' own error).
 template <int MODE>
-__device__ __forceinline__ bool dm_bf_pair(const float zf, const float A0r, const float A0i, const float A1r, const float A1i,
+__device__ __forceinline__ void dm_bf_pair(const float zf, const float A0r, const float A0i, const float A1r, const float A1i,
                                            const float A2r, const float A2i, const float prow, const float qrow,
                                            const float omrow, const float dpz, const float dqz, const float dmz,
-                                           const float tau_k, DmBfRow& rs)
+                                           const float tau_k, DmBfRow& rs, uint32_t& flags, const uint32_t bit)
 {
     const float p = fmaf(zf, dpz, prow), q = fmaf(zf, dqz, qrow), r = q - p;
     const float pqr = (p * q) * r;
@@ -189,8 +191,8 @@ __device__ __forceinline__ bool dm_bf_pair(const float zf, const float A0r, cons
     // this triangle on this row (tau_b, larger for a triangle that is coarse for the grid)
     const float m1 = fminf(fminf(fabsf(p), fabsf(q)), fabsf(r));
     const float m3 = fmaxf(fmaxf(fabsf(p), fabsf(q)), fabsf(r));
-    const bool bad = !(m1 * fabsf(pqr) > tau_k * m3);
-    const float R = bad ? 0.f : dm_rcp_approx(pqr);
+    const float lhs = m1 * fabsf(pqr), rhs = tau_k * m3;     // good = lhs > rhs
+    const float R = dm_rcp_approx(pqr);                      // inf / NaN for an excluded pair: never accumulated
     const float c0 = -r * R, c1 = q * R, c2 = -p * R;
     const float c0s = c0 * c0, c1s = c1 * c1, c2s = c2 * c2;
     const float d01r = A0r - A1r, d21r = A2r - A1r;
@@ -205,42 +207,106 @@ __device__ __forceinline__ bool dm_bf_pair(const float zf, const float A0r, cons
         sI *= om;
         sb *= om;
         sc *= om;
-        rs.T0 = fmaf(zf, s0, rs.T0);
+        asm("{\n\t.reg .pred g;\n\tsetp.gt.f32 g, %9, %10;\n\t"
+            "@g add.f32 %0, %0, %11;\n\t@g fma.rn.f32 %1, %15, %11, %1;\n\t"
+            "@g add.f32 %2, %2, %12;\n\t@g fma.rn.f32 %3, %15, %12, %3;\n\t"
+            "@g add.f32 %4, %4, %13;\n\t@g fma.rn.f32 %5, %15, %13, %5;\n\t"
+            "@g add.f32 %6, %6, %14;\n\t@g fma.rn.f32 %7, %15, %14, %7;\n\t"
+            "@!g or.b32 %8, %8, %16;\n\t}"
+            : "+f"(rs.S0), "+f"(rs.T0), "+f"(rs.SI), "+f"(rs.TI), "+f"(rs.SB), "+f"(rs.TB), "+f"(rs.SC), "+f"(rs.TC), "+r"(flags)
+            : "f"(lhs), "f"(rhs), "f"(s0), "f"(sI), "f"(sb), "f"(sc), "f"(zf), "r"(bit));
+    } else {
+        asm("{\n\t.reg .pred g;\n\tsetp.gt.f32 g, %8, %9;\n\t"
+            "@g add.f32 %0, %0, %10;\n\t"
+            "@g add.f32 %1, %1, %11;\n\t@g fma.rn.f32 %2, %14, %11, %2;\n\t"
+            "@g add.f32 %3, %3, %12;\n\t@g fma.rn.f32 %4, %14, %12, %4;\n\t"
+            "@g add.f32 %5, %5, %13;\n\t@g fma.rn.f32 %6, %14, %13, %6;\n\t"
+            "@!g or.b32 %7, %7, %15;\n\t}"
+            : "+f"(rs.S0), "+f"(rs.SI), "+f"(rs.TI), "+f"(rs.SB), "+f"(rs.TB), "+f"(rs.SC), "+f"(rs.TC), "+r"(flags)
+            : "f"(lhs), "f"(rhs), "f"(s0), "f"(sI), "f"(sb), "f"(sc), "f"(zf), "r"(bit));
     }
-    rs.S0 += s0;
-    rs.SI += sI;
-    rs.TI = fmaf(zf, sI, rs.TI);
-    rs.SB += sb;
-    rs.TB = fmaf(zf, sb, rs.TB);
-    rs.SC += sc;
-    rs.TC = fmaf(zf, sc, rs.TC);
-    return bad;
 }
 
-// One round of the pooled slow path: the n (<= 32) oldest queued pairs of the warp, one per lane whatever its owner.
-template <int MODE>
-__device__ __forceinline__ void dm_bf_round(DmBfWarp& W, const int lane, const int n, const int qh, const DmGridDev& grid,
-                                            const int ix_begin, const int row_begin, const float2* __restrict__ kappa)
+// position of the k-th (0-based) set bit of w (k < popc(w))
+__device__ __forceinline__ int dm_nth_set_bit(uint32_t w, int k)
 {
+    int pos = 0;
+#pragma unroll
+    for (int h = 16; h > 0; h >>= 1) {
+        const int c = __popc(w & ((1u << h) - 1u));
+        const bool up = k >= c;
+        k -= up ? c : 0;
+        pos += up ? h : 0;
+        w = up ? (w >> h) : w;
+    }
+    return pos;
+}
+
+// Queue of the pooled slow path (all warp-uniform): wh = ring position of the oldest flag word, wn = flag words queued,
+// count = flagged pairs queued, skip = pairs of the oldest word already evaluated.
+struct DmBfQueue {
+    int wh, wn, count, skip;
+};
+
+// One round of the pooled slow path: the n (<= 32) oldest queued pairs of the warp, one per lane whatever its owner.
+// Lane l looks at the l-th queued flag word; a prefix sum of the words' bit counts tells lane e which word and which of
+// its bits is pair e.  The results of one (row, owner) run are summed by a segmented scan and handed to the owner lane,
+// which adds them, weighted with the run's k_x, k_y, to its 13 sums acc[] -- in queue order (reading R22).
+// kbase = kappa of (row_begin, z = 0).
+template <int MODE>
+__device__ __forceinline__ void dm_bf_round(DmBfWarp& W, const int lane, const int n, DmBfQueue& Q, const DmGridDev& grid,
+                                            const float2* __restrict__ kbase, float (&acc)[DM_BWD_NSUM])
+{
+    const uint32_t full = 0xffffffffu;
+    uint4 ent = make_uint4(0u, 0u, 0u, 0u);
+    if (lane < Q.wn) ent = W.wq[(Q.wh + lane) & (DM_BF_QCAP - 1)];
+    const int cnt = __popc(ent.y) - (lane == 0 ? Q.skip : 0);
+    int off = cnt;  // inclusive prefix sum of the pairs per word
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(full, off, o);
+        if (lane >= o) off += t;
+    }
     const bool have = lane < n;
-    const uint32_t code = W.q[(qh + lane) & (DM_BF_QCAP - 1)];
-    const int z = (int)(code & 4095u), own = have ? (int)((code >> 12) & 31u) : 0;
-    const int row = row_begin + (have ? (int)(code >> 17) : 0);
-    const int ix = ix_begin + row / grid.ny, iy = row % grid.ny;
-    const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
-    const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny, kz = grid.kstep[2] * z;
+    int src = 0;    // the word that holds pair `lane` = number of words whose inclusive sum is <= lane
+#pragma unroll
+    for (int st = 16; st > 0; st >>= 1) {
+        const int t = __shfl_sync(full, off, src + st - 1);
+        if (t <= lane) src += st;
+    }
+    src = have ? src : 0;
+    const int s_first = __shfl_sync(full, off - cnt, src);        // index of the word's first unevaluated pair
+    const uint32_t s_base = __shfl_sync(full, ent.x, src), s_word = __shfl_sync(full, ent.y, src),
+                   s_freq = __shfl_sync(full, ent.z, src);
+    const int kbit = have ? lane - s_first + (src == 0 ? Q.skip : 0) : 0;
+    const uint32_t code = s_base + (uint32_t)dm_nth_set_bit(s_word, kbit);
+    // consume: whole words whose pairs are all in this round; the next word may be evaluated in part
+    {
+        const int n_done = __popc(__ballot_sync(full, lane < Q.wn && off <= n));
+        const int first_nd = __shfl_sync(full, off - cnt, n_done & 31);   // first pair index of the first word not finished
+        int skip = 0;
+        if (n_done < Q.wn && n_done < 32 && first_nd < n) skip = n - first_nd + (n_done == 0 ? Q.skip : 0);
+        Q.wh = (Q.wh + n_done) & (DM_BF_QCAP - 1);
+        Q.wn -= n_done;
+        Q.count -= n;
+        Q.skip = skip;
+    }
+    const int z = (int)(code & 4095u), own = (int)((code >> 12) & 31u);
+    const int rowl = (int)(code >> 17);
+    const int nx = (int)(short)(s_freq & 0xffffu), ny = (int)(short)(s_freq >> 16);
+    const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny, kz = grid.kstep[2] * (float)z;
     const float4* orc = W.rec + own * DM_BF_TREC;
     const float4 q0 = orc[0], q3 = orc[1], q4 = orc[2];
     const float p = fmaf(kz, q3.z, fmaf(kx, q3.x, ky * q3.y));
     const float q = fmaf(kz, q4.z, fmaf(kx, q4.x, ky * q4.y));
     const bool series = fmaxf(fmaxf(fabsf(p), fabsf(q)), fabsf(q - p)) < DM_SERIES_RADIUS;
     cf psi = {0.f, 0.f}, dp = {0.f, 0.f}, dq = {0.f, 0.f};
-    if (__any_sync(0xffffffffu, have && series)) {
+    if (__any_sync(full, have && series)) {
         cf a, b, c;
         dm_psi_series<true>(series ? p : 0.f, series ? q : 0.f, a, b, c);
         if (series) { psi = a; dp = b; dq = c; }
     }
-    if (__any_sync(0xffffffffu, have && !series)) {
+    if (__any_sync(full, have && !series)) {
         cf a, b, c;
         dm_psi_far_uniform(series ? 0.f : p, series ? 1.f : q, a, b, c);
         if (!series) { psi = a; dp = b; dq = c; }
@@ -248,7 +314,7 @@ __device__ __forceinline__ void dm_bf_round(DmBfWarp& W, const int lane, const i
     const cf E = dm_expmi_turns_fast(dm_phase_turns(nx, ny, z, __float_as_uint(q0.x), __float_as_uint(q0.y),
                                                     __float_as_uint(q0.z)));
     float2 kk = make_float2(0.f, 0.f);
-    if (have) kk = kappa[((size_t)ix * grid.ny + iy) * grid.nzh + z];
+    if (have) kk = kbase[(size_t)rowl * grid.nzh + z];
     const cf kE = cmul(cf{kk.x, kk.y}, E);
     const cf kg = cmul(kE, psi);
     // v[0..3] = s0, sI, sb, sc (the last three weighted with omega in volume mode), v[4..7] = k_z times them
@@ -268,67 +334,78 @@ __device__ __forceinline__ void dm_bf_round(DmBfWarp& W, const int lane, const i
     for (int i = 0; i < 4; ++i) v[4 + i] = kz * v[i];
     // segmented inclusive scan over the runs of equal (row, owner): head flags from adjacent keys
     const uint32_t key = have ? (code >> 12) : (0xffffff00u | (uint32_t)lane);
-    const uint32_t kprev = __shfl_up_sync(0xffffffffu, key, 1);
-    const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || kprev != key);
-    const int dist = lane - (31 - __clz((int)(heads & (0xffffffffu >> (31 - lane)))));   // distance to the run's first lane
+    const uint32_t kprev = __shfl_up_sync(full, key, 1);
+    const uint32_t heads = __ballot_sync(full, lane == 0 || kprev != key);
+    const int dist = lane - (31 - __clz((int)(heads & (full >> (31 - lane)))));   // distance to the run's first lane
+    const int maxdist = __reduce_max_sync(full, dist);
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
+        if (o <= maxdist) {   // warp-uniform: most rounds hold short runs only
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            if (MODE == 1 && i == 4) continue;  // k_z s0 is a volume-mode sum
-            const float x = __shfl_up_sync(0xffffffffu, v[i], o);
-            if (o <= dist) v[i] += x;
+            for (int i = 0; i < 8; ++i) {
+                if (MODE == 1 && i == 4) continue;  // k_z s0 is a volume-mode sum
+                const float x = __shfl_up_sync(full, v[i], o);
+                if (o <= dist) v[i] += x;
+            }
         }
     }
-    const bool end = have && (lane == 31 || ((heads >> (lane + 1)) & 1u));
-    // two runs of one owner (different rows) can end in the same round: they add in queue order, one rank at a time
-    const uint32_t endmask = __ballot_sync(0xffffffffu, end);
-    int rank = 0;
-    if (end) rank = __popc(__match_any_sync(endmask, own) & ((1u << lane) - 1u));
-    const int maxrank = __reduce_max_sync(0xffffffffu, rank);
-    for (int rk = 0; rk <= maxrank; ++rk) {
-        if (end && rank == rk) {
+    // hand every run's sums to its owner lane.  Two runs of one owner (different rows or chunks) can end in the same
+    // round: the lowest lane goes first (atomicMin), the others in later passes -- queue order.
+    bool pending = have && (lane == 31 || ((heads >> (lane + 1)) & 1u));
+    do {
+        W.src[lane] = 255;
+        __syncwarp();
+        if (pending) atomicMin(&W.src[own], lane);
+        __syncwarp();
+        const int s = W.src[lane];
+        if (pending && W.src[own] == lane) pending = false;
+        const bool got = s < 32;
+        const int sl = got ? s : 0;
+        const float gkx = __shfl_sync(full, kx, sl), gky = __shfl_sync(full, ky, sl);
+        float g[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (MODE == 1 && i == 4) continue;
+            g[i] = __shfl_sync(full, v[i], sl);
+        }
+        if (got) {
             if (MODE == 1) {
-                W.wacc[0][own] += v[0];
+                acc[0] += g[0];
             } else {
-                W.wacc[1][own] = fmaf(kx, v[0], W.wacc[1][own]);
-                W.wacc[2][own] = fmaf(ky, v[0], W.wacc[2][own]);
-                W.wacc[3][own] += v[4];
+                acc[1] = fmaf(gkx, g[0], acc[1]);
+                acc[2] = fmaf(gky, g[0], acc[2]);
+                acc[3] += g[4];
             }
 #pragma unroll
             for (int i = 1; i < 4; ++i) {
-                W.wacc[1 + 3 * i][own] = fmaf(kx, v[i], W.wacc[1 + 3 * i][own]);
-                W.wacc[2 + 3 * i][own] = fmaf(ky, v[i], W.wacc[2 + 3 * i][own]);
-                W.wacc[3 + 3 * i][own] += v[4 + i];
+                acc[1 + 3 * i] = fmaf(gkx, g[i], acc[1 + 3 * i]);
+                acc[2 + 3 * i] = fmaf(gky, g[i], acc[2 + 3 * i]);
+                acc[3 + 3 * i] += g[4 + i];
             }
         }
         __syncwarp();
-    }
+    } while (__any_sync(full, pending));
 }
 
 // ---- A6 backward, fast kernel -----------------------------------------------------------------------------------
-// grid = (n_lanes / DM_BF_THREADS, n_split): one warp per patch; part[(split*13 + s)*n_faces + face] as in
+// grid = (n_patches, n_split), one warp per CTA = one patch; part[(split*13 + s)*n_faces + face] as in
 // dm_k_backward_robust.  BAND = the narrow band is set (band_z holds the in-band z interval of every row).
 // SEG = frequencies between exact phase seeds (8, 16 or 32), n_tab <= DM_BF_NTAB_MAX the seed-table entries per vertex
 // slot (a super-segment is (n_tab + 1) SEG frequencies); both chosen by the host.  rows_per_split <= 32768.
-// Dynamic shared memory: n_tab * DM_BF_THREADS float2, ztab[a][tid] = e^{-2 pi i ((a+1) SEG) u_z} of the thread's vertex
-// slot: with the exact super-segment phase a phase is never more than SEG-1 fp32 rotations away from an exact value.
 template <int MODE, int SEG, bool BAND>
-__global__ void __launch_bounds__(DM_BF_THREADS, DM_BF_MINCTA)
+__global__ void __launch_bounds__(32, DM_BF_MINCTA)
 dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__ vrec_g, DmPatchDev pt, int n_faces,
                    DmGridDev grid, int ix_begin, int ix_end, int rows_per_split, float tau_b, int n_tab,
                    const float2* __restrict__ kappa, const int2* __restrict__ band_z, float* __restrict__ part)
 {
     static_assert(SEG == 8 || SEG == 16 || SEG == 32, "SEG is a multiple of the stage and divides the chunk");
-    extern __shared__ float2 dm_bf_ztab[];
-    __shared__ DmBfWarp wsm[DM_BF_WARPS];
-    const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
-    DmBfWarp& W = wsm[wrp];
-    const int gl = blockIdx.x * DM_BF_THREADS + tid;       // global lane = 32 * patch + lane
+    __shared__ DmBfWarp W;
+    const int lane = threadIdx.x;
+    const int gl = blockIdx.x * 32 + lane;                 // global lane = 32 * patch + lane
     const int face = pt.face[gl];
     const bool live = face >= 0;
     float dpz, dqz, dmz;
-    int l0, l1, l2;
+    const float4 *pa0, *pa1, *pa2;                         // the staged phases of the triangle's corners
     {
         const float4 r0 = trec_g[(size_t)DM_BF_TREC * gl], r1 = trec_g[(size_t)DM_BF_TREC * gl + 1],
                      r2 = trec_g[(size_t)DM_BF_TREC * gl + 2], r3 = trec_g[(size_t)DM_BF_TREC * gl + 3];
@@ -337,7 +414,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         W.rec[lane * DM_BF_TREC + 2] = r2;
         W.rec[lane * DM_BF_TREC + 3] = r3;
         const uint32_t loc = __float_as_uint(r0.w);
-        l0 = (int)(loc & 255u), l1 = (int)((loc >> 8) & 255u), l2 = (int)((loc >> 16) & 255u);
+        pa0 = &W.at4[0][loc & 255u], pa1 = &W.at4[0][(loc >> 8) & 255u], pa2 = &W.at4[0][(loc >> 16) & 255u];
         dpz = grid.kstep[2] * r1.z, dqz = grid.kstep[2] * r2.z, dmz = grid.kstep[2] * r3.z;
     }
     // the vertex slot this lane owns (slot lane of its patch)
@@ -350,20 +427,18 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
     const int row_end = min(n_rows, row_begin + rows_per_split);
     const int SS = (n_tab + 1) * SEG;                      // frequencies per super-segment
 
-    // seed table (row-independent): exact z-phases of this thread's vertex slot at the multiples of SEG
+    // seed table (row-independent): exact z-phases of this lane's vertex slot at the multiples of SEG
     for (int a = 0; a < n_tab; ++a) {
         const cf z0 = dm_expmi_turns((uint32_t)((a + 1) * SEG) * uaz);
-        dm_bf_ztab[a * DM_BF_THREADS + tid] = make_float2(z0.re, z0.im);
+        W.ztab[a][lane] = make_float2(z0.re, z0.im);
     }
-#pragma unroll
-    for (int s = 0; s < DM_BWD_NSUM; ++s) W.wacc[s][lane] = 0.f;
     __syncwarp();
 
     // acc: [0] S0 | [1..3] Q | [4..6] W | [7..9] Vb | [10..12] Vc   (dm_k_backward_robust)
     float acc[DM_BWD_NSUM];
 #pragma unroll
     for (int s = 0; s < DM_BWD_NSUM; ++s) acc[s] = 0.f;
-    int qh = 0, qlen = 0;                                  // ring buffer of flagged pairs (warp-uniform)
+    DmBfQueue Q = {0, 0, 0, 0};                            // flag words waiting for the pooled path (warp-uniform)
 
     // in-band z interval of a row, started at a seed position (the whole row without a band)
     auto row_range = [&](int row, int& lo, int& hi) {
@@ -374,7 +449,8 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
             hi = bz.y;
         }
     };
-    const float2* krow = kappa + ((size_t)ix_begin * grid.ny + row_begin) * nzh;
+    const float2* const kbase = kappa + ((size_t)ix_begin * grid.ny + row_begin) * nzh;
+    const float2* krow = kbase;
     float2 knext = make_float2(0.f, 0.f);                  // kappa of this lane's frequency of the NEXT chunk
     int pref_row = -1;                                     // row whose first chunk knext holds
     int ix = ix_begin + row_begin / grid.ny, iy = row_begin % grid.ny;
@@ -387,6 +463,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         const int nx = dm_signed_freq(ix, grid.nx), ny = dm_signed_freq(iy, grid.ny);
         if (++iy == grid.ny) iy = 0, ++ix;
         if (z_lo >= z_hi) continue;
+        const int rowl = row - row_begin;
         const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny;
         float prow, qrow, omrow, tau_row;
         {
@@ -403,17 +480,23 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         if (pref_row != row) knext = (z_lo + lane < z_hi) ? krow[z_lo + lane] : make_float2(0.f, 0.f);
         DmBfRow rs = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         cf Xs = {1.f, 0.f}, Ea = {1.f, 0.f};
-        int zs = z_lo;
+        int zs = z_lo, ze = z_lo;                          // current super-segment [zs, ze)
+        const float2* ztp = &W.ztab[0][lane];              // next seed-table entry of the super-segment
         for (int z = z_lo; z < z_hi;) {
-            if (z == zs) Xs = dm_expmi_turns(xturns + (uint32_t)zs * uaz);   // exact phase at the super-segment start
-            const int ze = min(zs + SS, z_hi);
+            if (z == ze) {                                 // a new super-segment: exact phase at its start
+                zs = z;
+                ze = min(zs + SS, z_hi);
+                Xs = dm_expmi_turns(xturns + (uint32_t)zs * uaz);
+                Ea = Xs;
+                ztp = &W.ztab[0][lane];
+            }
             const int clen = min(DM_BF_CHUNK, ze - z);
-            // ---- stage kappa of the chunk, prefetch the next chunk's ------------------------------------------------
+            // ---- stage kappa of the chunk, prefetch the next chunk's (entries past its end are loaded, never read) ----
             W.kbuf[lane] = knext;
             __syncwarp();
             {
                 const int zn = z + clen;
-                if (zn < z_hi) {          // (entries past the next chunk's end are loaded but never read)
+                if (zn < z_hi) {
                     knext = (zn + lane < z_hi) ? krow[zn + lane] : make_float2(0.f, 0.f);
                 } else if (zn_lo < zn_hi) {
                     knext = (zn_lo + lane < zn_hi) ? krow[nzh + zn_lo + lane] : make_float2(0.f, 0.f);
@@ -422,95 +505,75 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
             }
             // ---- fast pass over the chunk: bodies of DM_BF_STAGE frequencies, exact seeds every SEG -----------------
             uint32_t word = 0;
+            float zf = (float)z;
+            const float4* kb4 = reinterpret_cast<const float4*>(W.kbuf);
             int zloc = 0;
 #pragma unroll 1
-            for (; zloc < clen; zloc += DM_BF_STAGE) {
-                const int z0 = z + zloc;
-                if (((z0 - zs) & (SEG - 1)) == 0) {   // exact seed
-                    Ea = Xs;
-                    if (z0 > zs) {
-                        const float2 a0 = dm_bf_ztab[((z0 - zs) / SEG - 1) * DM_BF_THREADS + tid];
-                        Ea = cmul(Xs, cf{a0.x, a0.y});
-                    }
+            for (; zloc + DM_BF_STAGE <= clen; zloc += DM_BF_STAGE, zf += (float)DM_BF_STAGE, kb4 += DM_BF_STAGE / 2) {
+                if ((SEG == DM_BF_STAGE || ((z + zloc - zs) & (SEG - 1)) == 0) && z + zloc != zs) {   // exact seed
+                    const float2 a0 = *ztp;
+                    ztp += 32;
+                    Ea = cmul(Xs, cf{a0.x, a0.y});
                 }
-                const float zf = (float)z0;
+                // every lane writes A_v of its vertex slot for 8 frequencies, then evaluates its triangle at them
+#pragma unroll
+                for (int jp = 0; jp < DM_BF_STAGE / 2; ++jp) {
+                    const float4 k4 = kb4[jp];
+                    const cf A = cmul(cf{k4.x, k4.y}, Ea);
+                    Ea = cmul(Ea, rhoa);
+                    const cf B = cmul(cf{k4.z, k4.w}, Ea);
+                    Ea = cmul(Ea, rhoa);
+                    W.at4[jp][lane] = make_float4(A.re, A.im, B.re, B.im);
+                }
+                __syncwarp();
                 uint32_t sf = 0;
-                if (zloc + DM_BF_STAGE <= clen) {
-                    // every lane writes A_v of its vertex slot for 8 frequencies, then evaluates its triangle at them
-                    const float4* kb4 = reinterpret_cast<const float4*>(W.kbuf) + (zloc >> 1);
 #pragma unroll
-                    for (int jp = 0; jp < DM_BF_STAGE / 2; ++jp) {
-                        const float4 k4 = kb4[jp];
-                        const cf A = cmul(cf{k4.x, k4.y}, Ea);
-                        Ea = cmul(Ea, rhoa);
-                        const cf B = cmul(cf{k4.z, k4.w}, Ea);
-                        Ea = cmul(Ea, rhoa);
-                        W.at4[jp][lane] = make_float4(A.re, A.im, B.re, B.im);
-                    }
-                    __syncwarp();
-#pragma unroll
-                    for (int jp = 0; jp < DM_BF_STAGE / 2; ++jp) {
-                        const float4 a0 = W.at4[jp][l0], a1 = W.at4[jp][l1], a2 = W.at4[jp][l2];
-                        if (dm_bf_pair<MODE>(zf + (float)(2 * jp), a0.x, a0.y, a1.x, a1.y, a2.x, a2.y, prow, qrow, omrow, dpz, dqz,
-                                             dmz, tau_row, rs))
-                            sf |= 1u << (2 * jp);
-                        if (dm_bf_pair<MODE>(zf + (float)(2 * jp + 1), a0.z, a0.w, a1.z, a1.w, a2.z, a2.w, prow, qrow, omrow, dpz,
-                                             dqz, dmz, tau_row, rs))
-                            sf |= 1u << (2 * jp + 1);
-                    }
-                    __syncwarp();
-                } else {
-                    // ragged end of the chunk: one frequency at a time
-#pragma unroll 1
-                    for (int j = 0; zloc + j < clen; ++j) {
-                        const float2 k1 = W.kbuf[zloc + j];
-                        const cf A = cmul(cf{k1.x, k1.y}, Ea);
-                        Ea = cmul(Ea, rhoa);
-                        W.at4[0][lane] = make_float4(A.re, A.im, 0.f, 0.f);
-                        __syncwarp();
-                        const float4 a0 = W.at4[0][l0], a1 = W.at4[0][l1], a2 = W.at4[0][l2];
-                        if (dm_bf_pair<MODE>(zf + (float)j, a0.x, a0.y, a1.x, a1.y, a2.x, a2.y, prow, qrow, omrow, dpz, dqz, dmz,
-                                             tau_row, rs))
-                            sf |= 1u << j;
-                        __syncwarp();
-                    }
+                for (int jp = 0; jp < DM_BF_STAGE / 2; ++jp) {
+                    const float4 a0 = pa0[jp * DM_PATCH_MAXV], a1 = pa1[jp * DM_PATCH_MAXV], a2 = pa2[jp * DM_PATCH_MAXV];
+                    dm_bf_pair<MODE>(zf + (float)(2 * jp), a0.x, a0.y, a1.x, a1.y, a2.x, a2.y, prow, qrow, omrow, dpz, dqz, dmz,
+                                     tau_row, rs, sf, 1u << (2 * jp));
+                    dm_bf_pair<MODE>(zf + (float)(2 * jp + 1), a0.z, a0.w, a1.z, a1.w, a2.z, a2.w, prow, qrow, omrow, dpz, dqz,
+                                     dmz, tau_row, rs, sf, 1u << (2 * jp + 1));
                 }
+                __syncwarp();
                 word |= sf << zloc;
             }
-            word = live ? word : 0u;
-            // ---- queue the flagged pairs of the chunk in (lane, frequency) order; evaluate whole rounds of 32 ---------
-            int cnt = __popc(word);
-            if (__any_sync(0xffffffffu, cnt != 0)) {
-                const uint32_t base = ((uint32_t)(row - row_begin) << 17) | ((uint32_t)lane << 12) | (uint32_t)z;
-                for (;;) {
-                    int off = cnt;  // inclusive prefix sum over lanes
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int n = __shfl_up_sync(0xffffffffu, off, o);
-                        if (lane >= o) off += n;
-                    }
-                    const int total = __shfl_sync(0xffffffffu, off, 31);
-                    const int room = DM_BF_QCAP - qlen;
-                    int pos = off - cnt;
-                    while (word != 0u && pos < room) {
-                        const int j = __ffs(word) - 1;
-                        word &= word - 1;
-                        W.q[(qh + qlen + pos) & (DM_BF_QCAP - 1)] = base + (uint32_t)j;
-                        ++pos;
-                    }
-                    qlen += min(total, room);
+            if (zloc < clen) {
+                // ragged end of the chunk: one frequency at a time (it starts at a stage boundary: maybe a seed)
+                if (((z + zloc - zs) & (SEG - 1)) == 0 && z + zloc != zs) {
+                    const float2 a0 = *ztp;
+                    ztp += 32;
+                    Ea = cmul(Xs, cf{a0.x, a0.y});
+                }
+#pragma unroll 1
+                for (; zloc < clen; ++zloc, zf += 1.0f) {
+                    const float2 k1 = W.kbuf[zloc];
+                    const cf A = cmul(cf{k1.x, k1.y}, Ea);
+                    Ea = cmul(Ea, rhoa);
+                    W.at4[0][lane] = make_float4(A.re, A.im, 0.f, 0.f);
                     __syncwarp();
-                    while (qlen >= 32) {
-                        dm_bf_round<MODE>(W, lane, 32, qh, grid, ix_begin, row_begin, kappa);
-                        qh = (qh + 32) & (DM_BF_QCAP - 1);
-                        qlen -= 32;
-                    }
-                    if (total <= room) break;
-                    cnt = __popc(word);
+                    const float4 a0 = pa0[0], a1 = pa1[0], a2 = pa2[0];
+                    dm_bf_pair<MODE>(zf, a0.x, a0.y, a1.x, a1.y, a2.x, a2.y, prow, qrow, omrow, dpz, dqz, dmz, tau_row, rs, word,
+                                     1u << zloc);
+                    __syncwarp();
+                }
+            }
+            word = live ? word : 0u;
+            // ---- queue the chunk's flag words in lane order; evaluate whole rounds of 32 pairs ------------------------
+            {
+                const uint32_t m = __ballot_sync(0xffffffffu, word != 0u);
+                if (m != 0u) {
+                    if (word != 0u)
+                        W.wq[(Q.wh + Q.wn + __popc(m & ((1u << lane) - 1u))) & (DM_BF_QCAP - 1)] =
+                            make_uint4(((uint32_t)rowl << 17) | ((uint32_t)lane << 12) | (uint32_t)z, word,
+                                       ((uint32_t)nx & 0xffffu) | ((uint32_t)ny << 16), 0u);
+                    Q.wn += __popc(m);
+                    Q.count += __reduce_add_sync(0xffffffffu, __popc(word));
+                    __syncwarp();
+                    while (Q.count >= 32) dm_bf_round<MODE>(W, lane, 32, Q, grid, kbase, acc);
                 }
             }
             z += clen;
-            if (z == ze) zs = ze;
         }
         // fold the row into the 13 sums (the z-weighted sums carry the z index: k_z = kstep_z z)
         if (MODE == 1) {
@@ -530,12 +593,9 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
         acc[11] = fmaf(ky, rs.SC, acc[11]);
         acc[12] = fmaf(grid.kstep[2], rs.TC, acc[12]);
     }
-    // the pairs still queued (< 32), then the pooled path's sums
-    if (qlen > 0) dm_bf_round<MODE>(W, lane, qlen, qh, grid, ix_begin, row_begin, kappa);
-    __syncwarp();
+    if (Q.count > 0) dm_bf_round<MODE>(W, lane, Q.count, Q, grid, kbase, acc);   // the pairs still queued (< 32)
     if (live) {
 #pragma unroll
-        for (int s = 0; s < DM_BWD_NSUM; ++s)
-            part[((size_t)blockIdx.y * DM_BWD_NSUM + s) * n_faces + face] = acc[s] + W.wacc[s][lane];
+        for (int s = 0; s < DM_BWD_NSUM; ++s) part[((size_t)blockIdx.y * DM_BWD_NSUM + s) * n_faces + face] = acc[s];
     }
 }
