@@ -49,7 +49,9 @@
 #define DM_BF_MINCTA 20        // resident CTAs (= warps) per SM the register allocation aims at (<= 102 registers)
 #endif
 #define DM_BF_CHUNK 32          // frequencies per chunk = one flag word per thread
-#define DM_BF_STAGE 8           // frequencies whose vertex phases are staged in shared memory at a time
+#ifndef DM_BF_STAGE
+#define DM_BF_STAGE 8
+#endif                          // frequencies whose vertex phases are staged in shared memory at a time
 #define DM_BF_NTAB_MAX 8        // seed-table entries per vertex slot: a super-segment is (n_tab + 1) * SEG frequencies
 #define DM_BF_QCAP 64           // ring buffer of flag words per warp: < 32 carried over + <= 32 new per chunk
 #define DM_BF_TREC 4            // float4 per triangle record
@@ -268,13 +270,10 @@ __device__ __forceinline__ void dm_bf_round(DmBfWarp& W, const int lane, const i
         if (lane >= o) off += t;
     }
     const bool have = lane < n;
-    int src = 0;    // the word that holds pair `lane` = number of words whose inclusive sum is <= lane
-#pragma unroll
-    for (int st = 16; st > 0; st >>= 1) {
-        const int t = __shfl_sync(full, off, src + st - 1);
-        if (t <= lane) src += st;
-    }
-    src = have ? src : 0;
+    // the word that holds pair `lane`: every queued word holds at least one pair, so it is the number of words that start
+    // at or before the pair, minus one
+    const uint32_t starts = __reduce_or_sync(full, (lane < Q.wn && off - cnt < 32) ? (1u << (off - cnt)) : 0u);
+    const int src = have ? __popc(starts & (full >> (31 - lane))) - 1 : 0;
     const int s_first = __shfl_sync(full, off - cnt, src);        // index of the word's first unevaluated pair
     const uint32_t s_base = __shfl_sync(full, ent.x, src), s_word = __shfl_sync(full, ent.y, src),
                    s_freq = __shfl_sync(full, ent.z, src);
@@ -293,6 +292,8 @@ __device__ __forceinline__ void dm_bf_round(DmBfWarp& W, const int lane, const i
     }
     const int z = (int)(code & 4095u), own = (int)((code >> 12) & 31u);
     const int rowl = (int)(code >> 17);
+    float2 kk = make_float2(0.f, 0.f);                     // (issued early: an L2 access)
+    if (have) kk = kbase[(size_t)rowl * grid.nzh + z];
     const int nx = (int)(short)(s_freq & 0xffffu), ny = (int)(short)(s_freq >> 16);
     const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * ny, kz = grid.kstep[2] * (float)z;
     const float4* orc = W.rec + own * DM_BF_TREC;
@@ -313,8 +314,6 @@ __device__ __forceinline__ void dm_bf_round(DmBfWarp& W, const int lane, const i
     }
     const cf E = dm_expmi_turns_fast(dm_phase_turns(nx, ny, z, __float_as_uint(q0.x), __float_as_uint(q0.y),
                                                     __float_as_uint(q0.z)));
-    float2 kk = make_float2(0.f, 0.f);
-    if (have) kk = kbase[(size_t)rowl * grid.nzh + z];
     const cf kE = cmul(cf{kk.x, kk.y}, E);
     const cf kg = cmul(kE, psi);
     // v[0..3] = s0, sI, sb, sc (the last three weighted with omega in volume mode), v[4..7] = k_z times them
@@ -510,7 +509,7 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
             int zloc = 0;
 #pragma unroll 1
             for (; zloc + DM_BF_STAGE <= clen; zloc += DM_BF_STAGE, zf += (float)DM_BF_STAGE, kb4 += DM_BF_STAGE / 2) {
-                if ((SEG == DM_BF_STAGE || ((z + zloc - zs) & (SEG - 1)) == 0) && z + zloc != zs) {   // exact seed
+                if ((SEG <= DM_BF_STAGE || ((z + zloc - zs) & (SEG - 1)) == 0) && z + zloc != zs) {   // exact seed
                     const float2 a0 = *ztp;
                     ztp += 32;
                     Ea = cmul(Xs, cf{a0.x, a0.y});
@@ -518,6 +517,11 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
                 // every lane writes A_v of its vertex slot for 8 frequencies, then evaluates its triangle at them
 #pragma unroll
                 for (int jp = 0; jp < DM_BF_STAGE / 2; ++jp) {
+                    if (SEG < DM_BF_STAGE && jp > 0 && (2 * jp) % SEG == 0) {   // a seed inside the body
+                        const float2 a0 = *ztp;
+                        ztp += 32;
+                        Ea = cmul(Xs, cf{a0.x, a0.y});
+                    }
                     const float4 k4 = kb4[jp];
                     const cf A = cmul(cf{k4.x, k4.y}, Ea);
                     Ea = cmul(Ea, rhoa);
@@ -539,14 +543,14 @@ dm_k_backward_fast(const float4* __restrict__ trec_g, const float4* __restrict__
                 word |= sf << zloc;
             }
             if (zloc < clen) {
-                // ragged end of the chunk: one frequency at a time (it starts at a stage boundary: maybe a seed)
-                if (((z + zloc - zs) & (SEG - 1)) == 0 && z + zloc != zs) {
-                    const float2 a0 = *ztp;
-                    ztp += 32;
-                    Ea = cmul(Xs, cf{a0.x, a0.y});
-                }
+                // ragged end of the chunk: one frequency at a time
 #pragma unroll 1
                 for (; zloc < clen; ++zloc, zf += 1.0f) {
+                    if (((z + zloc - zs) & (SEG - 1)) == 0 && z + zloc != zs) {   // exact seed
+                        const float2 a0 = *ztp;
+                        ztp += 32;
+                        Ea = cmul(Xs, cf{a0.x, a0.y});
+                    }
                     const float2 k1 = W.kbuf[zloc];
                     const cf A = cmul(cf{k1.x, k1.y}, Ea);
                     Ea = cmul(Ea, rhoa);
