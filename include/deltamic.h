@@ -101,10 +101,17 @@ typedef enum dm_option {
     DM_OPT_TAU           = 2, /* forward: gap-product threshold |pqr| at or below which a pair leaves the fast path (>= 0) */
     DM_OPT_TAU_BWD       = 3, /* backward: threshold on m1^2 m2 (the two smallest |gaps|) below which a pair leaves
                                  the fast path                                                                     */
-    DM_OPT_AREA_NORMALISED = 4 /* DM_SURFACE only; 1 = the paper's membrane density u = F / |Lambda| (PAPER.md:177-186
+    DM_OPT_AREA_NORMALISED = 4, /* DM_SURFACE only; 1 = the paper's membrane density u = F / |Lambda| (PAPER.md:177-186
                                   eq. 12) and its gradient (eq. 13): forward divides by the total area, backward takes
                                   dL/du and adds the -(sum_k Re(conj(G) u)/|Lambda|) d|Lambda|/dv term (it recomputes
                                   the forward once).  Whole grid only (a slab returns DM_ERR_UNSUPPORTED).  Default 0. */
+    DM_OPT_REUSE_SPECTRUM = 5  /* 1 = the caller promises that every dm_render_backward is called with the vertices (and
+                                  PSF mode) of the LAST dm_render on this plan, with no other forward call, setter or
+                                  option change in between: the PSF-parameter gradient and eq. 13's extra term then take F
+                                  from the spectrum dm_render left in the plan instead of recomputing the forward mesh FT
+                                  (shape and PSF are fitted in the same loop).  The library cannot
+                                  check the vertices; it returns DM_ERR_INVALID_ARG when the plan holds no such spectrum
+                                  (no dm_render yet, or one of the calls above intervened).  Default 0 (recompute). */
 } dm_option;
 int dm_plan_set_option(dm_plan* plan, int option, double value);
 
@@ -126,6 +133,13 @@ int dm_mesh_ft_forward(dm_plan* plan, const float* vertices_dev, float* F_dev);
 int dm_mesh_ft_backward(dm_plan* plan, const float* vertices_dev, const float* dL_dF_dev,
                         float* dL_dvertices_dev);
 
+/* dm_mesh_ft_backward for a caller that still holds the spectrum dm_mesh_ft_forward returned for THESE vertices
+ * (F_dev, unchanged; the last forward call on the plan must have been that one): with DM_OPT_AREA_NORMALISED the
+ * sum_k Re(conj(G) u) of eq. 13 is taken with it instead of a recomputed forward.  Without that option F_dev is unused
+ * and the call equals dm_mesh_ft_backward. */
+int dm_mesh_ft_backward_with_spectrum(dm_plan* plan, const float* vertices_dev, const float* dL_dF_dev,
+                                      const float* F_dev, float* dL_dvertices_dev);
+
 /* Whole forward render: mesh FT, multiply by the PSF spectrum and the origin shift, inverse real FFT.
  *   psf_cov_host  6 floats on the HOST: covariance of the Gaussian PSF in physical units, order
  *                 xx, yy, zz, xy, xz, yz;  h_hat(k) = exp(-1/2 k^T Sigma k)  (eq. 4 with reading R5).
@@ -138,8 +152,9 @@ int dm_render(dm_plan* plan, const float* vertices_dev, const float* psf_cov_hos
  *   dL_dpsf_cov_host   NULL, or 6 floats on the HOST that receive dL/dSigma in the order of psf_cov_host
  *                      (the PSF parameters are fitted by gradient descent); an off-diagonal
  *                      entry is the derivative with respect to the one number that fills both symmetric positions.
- *                      When non-NULL the call recomputes the forward mesh FT of these vertices (one extra
- *                      dm_mesh_ft_forward) and SYNCHRONISES the stream before it returns. */
+ *                      When non-NULL the call needs the forward mesh FT of these vertices -- recomputed (one extra
+ *                      dm_mesh_ft_forward) unless DM_OPT_REUSE_SPECTRUM is set -- and SYNCHRONISES the stream before
+ *                      it returns (the six numbers land in host memory). */
 int dm_render_backward(dm_plan* plan, const float* vertices_dev, const float* psf_cov_host,
                        const float* dL_dimage_dev, float* dL_dvertices_dev, float* dL_dpsf_cov_host);
 

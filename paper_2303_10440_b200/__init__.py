@@ -9,6 +9,7 @@ from ._binding import (  # noqa: F401
     DM_OPT_AREA_NORMALISED,
     DM_OPT_BACKWARD_PATH,
     DM_OPT_FORWARD_PATH,
+    DM_OPT_REUSE_SPECTRUM,
     DM_OPT_TAU,
     DM_OPT_TAU_BWD,
     DM_SURFACE,

@@ -9,10 +9,11 @@ _LIB_PATH = os.path.join(HERE, "libdeltamic.so")
 
 DM_VOLUME, DM_SURFACE = 0, 1
 DM_OPT_FORWARD_PATH, DM_OPT_BACKWARD_PATH, DM_OPT_TAU, DM_OPT_TAU_BWD, DM_OPT_AREA_NORMALISED = 0, 1, 2, 3, 4
+DM_OPT_REUSE_SPECTRUM = 5
 
 # every symbol include/deltamic.h declares
 _SYMBOLS = (
-    "dm_plan_create", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_render",
+    "dm_plan_create", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_mesh_ft_backward_with_spectrum", "dm_render",
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
     "dm_plan_launch_count", "dm_plan_paths_used", "dm_plan_destroy", "dm_error_string", "dm_version",
 )
@@ -58,6 +59,7 @@ def load_library():
     lib.dm_plan_set_narrow_band.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_float]
     lib.dm_mesh_ft_forward.argtypes = [vp, fp, fp]
     lib.dm_mesh_ft_backward.argtypes = [vp, fp, fp, fp]
+    lib.dm_mesh_ft_backward_with_spectrum.argtypes = [vp, fp, fp, fp, fp]
     lib.dm_render.argtypes = [vp, fp, ctypes.POINTER(ctypes.c_float), fp]
     lib.dm_render_backward.argtypes = [vp, fp, ctypes.POINTER(ctypes.c_float), fp, fp, ctypes.POINTER(ctypes.c_float)]
     lib.dm_spectrum_to_image.argtypes = [vp, fp, ctypes.POINTER(ctypes.c_float), fp]
@@ -179,14 +181,20 @@ class Plan:
         _check(self._lib.dm_mesh_ft_forward(self._h, v.data_ptr(), o.data_ptr()), "dm_mesh_ft_forward")
         return out
 
-    def mesh_ft_backward(self, vertices, dL_dF, out=None):
+    def mesh_ft_backward(self, vertices, dL_dF, out=None, spectrum=None):
+        """``spectrum``: the F that mesh_ft_forward returned for these vertices (dm_mesh_ft_backward_with_spectrum)."""
         torch = self._torch
         v = self._vertices(vertices)
         g = self._f32(dL_dF, 2 * self._nk(), "dL_dF")
         if out is None:
             out = torch.empty((self.n_vertices, 3), dtype=torch.float32, device=self.device)
         o = self._f32(out, self.n_vertices * 3, "dL_dvertices")
-        _check(self._lib.dm_mesh_ft_backward(self._h, v.data_ptr(), g.data_ptr(), o.data_ptr()), "dm_mesh_ft_backward")
+        if spectrum is not None:
+            f = self._f32(spectrum, 2 * self._nk(), "F")
+            _check(self._lib.dm_mesh_ft_backward_with_spectrum(self._h, v.data_ptr(), g.data_ptr(), f.data_ptr(),
+                                                               o.data_ptr()), "dm_mesh_ft_backward_with_spectrum")
+        else:
+            _check(self._lib.dm_mesh_ft_backward(self._h, v.data_ptr(), g.data_ptr(), o.data_ptr()), "dm_mesh_ft_backward")
         return out
 
     def render(self, vertices, psf_cov, out=None):

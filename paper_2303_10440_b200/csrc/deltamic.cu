@@ -16,6 +16,9 @@
 #include "dm_strips.h"
 
 #define DM_VERSION 100
+#ifndef DM_BWD_SPLIT_TARGET
+#define DM_BWD_SPLIT_TARGET 192  // k-splits of the backward: (128-triangle blocks x splits) per SM
+#endif
 
 struct dm_plan {
     dm_grid grid;
@@ -39,7 +42,7 @@ struct dm_plan {
     float* part = nullptr;           // [n_split_max*13*n_faces]
     float* corner = nullptr;         // [n_faces*9]
     float2* spec = nullptr;          // [n_k] scratch spectrum (S, R or G)
-    float2* spec2 = nullptr;         // [n_k] F or G inside dm_render*
+    float2* spec2 = nullptr;         // [n_k] G inside dm_render_backward
     int n_split_max = 0;
     // strip walk of the fast forward kernel (topology only; built at create)
     int32_t *st_new = nullptr, *st_prev = nullptr, *st_ret = nullptr, *st_fid = nullptr, *st_chunk_off = nullptr;
@@ -62,7 +65,10 @@ struct dm_plan {
     int2* band_z = nullptr;          // [nx*ny] in-band z interval of every row (narrow band), valid while band_on
     bool band_on = false;
     float2* kappa = nullptr;         // [n_k] kappa(k) of the fast backward kernel (dm_k_kappa), allocated on first use
-    float2* spec3 = nullptr;         // [n_k] forward spectrum recomputed for the PSF gradient (allocated on first use)
+    float2* spec3 = nullptr;         // [n_k] the forward spectrum F of dm_render (kept for dm_render_backward), or the one
+                                     // recomputed for the PSF gradient / eq. 13 (allocated on first use)
+    bool F_valid = false;            // spec3 and dc_total belong to the last dm_render and nothing changed them since
+    bool reuse_F = false;            // DM_OPT_REUSE_SPECTRUM
     double* psfg_part = nullptr;     // [DM_PSFG_BLOCKS*6] block sums of the PSF gradient
     float* psfg_out = nullptr;       // [6] device result of the PSF gradient
     int fwd_path = 0, bwd_path = 0;  // 0 = fast, 1 = robust
@@ -113,7 +119,7 @@ int backward_splits(const dm_plan* p, int* rows_per_split)
     // enough (triangle-block x k-split) CTAs to fill the machine (5 CTAs per SM) about 10 times over: short tail
     const int n_rows = (p->ix_end - p->ix_begin) * p->gd.ny;
     const int tri_blocks = (p->n_faces + 127) / 128;
-    int want = (p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
+    int want = (p->n_sm * DM_BWD_SPLIT_TARGET + tri_blocks - 1) / tri_blocks;
     if (p->band_on) want = std::max(want, std::min(p->n_split_max, 64));   // rows differ in cost under the narrow band:
                                                                              // many small CTAs balance the load
     // a CTA sets up its seed table and records once: give it at least ~512 frequencies per triangle
@@ -207,14 +213,17 @@ int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
         dm_k_forward_fast<0><<<grid, DM_FAST_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->gd, p->ix_begin, p->ix_end,
                                                                       n_yruns, p->tau, p->hmax2, stride, p->fwd_part);
     if ((rc = check_launch(p))) return rc;
-    const int W = 2 * DM_LOWK_BOX + 1;
-    const unsigned lowk_blocks = (unsigned)(W * W * (DM_LOWK_BOX + 1));   // one CTA per frequency of the low-k box
+    // candidates of the low-k kernel: the part of its box that exists on this grid; a CTA strides over them and only
+    // the low ones (|k| h_max < DM_LOWK_RADIUS, decided on the device) cost anything
+    const int bx = std::min(DM_LOWK_BOX, p->gd.nx / 2), by = std::min(DM_LOWK_BOX, p->gd.ny / 2), bz = std::min(DM_LOWK_BOX, p->gd.nz / 2);
+    const long long n_cand = (long long)(2 * bx + 1) * (2 * by + 1) * (bz + 1);
+    const unsigned lowk_blocks = (unsigned)std::min<long long>(n_cand, (long long)p->n_sm * 8);
     if (p->mode == DM_SURFACE)
         dm_k_forward_lowk<1><<<lowk_blocks, DM_LOWK_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
-                                                                 p->ix_end, p->hmax2, (float2*)F_dev);
+                                                                 p->ix_end, bx, by, bz, p->hmax2, (float2*)F_dev);
     else
         dm_k_forward_lowk<0><<<lowk_blocks, DM_LOWK_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
-                                                                 p->ix_end, p->hmax2, (float2*)F_dev);
+                                                                 p->ix_end, bx, by, bz, p->hmax2, (float2*)F_dev);
     if ((rc = check_launch(p))) return rc;
     const long long n_slab = (long long)(p->ix_end - p->ix_begin) * p->gd.ny * p->gd.nzh;
     dm_k_forward_finish<<<(unsigned)((n_slab + 255) / 256), 256, 0, p->stream>>>(p->fwd_part, stride, p->st_n_chunks, p->gd,
@@ -248,7 +257,9 @@ int run_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
     return check_launch(p);
 }
 
-int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, float* dv_dev)
+// F_reuse: the (area-normalised) forward spectrum of these vertices when the caller already has it and dc_total still
+// holds their total area; nullptr = recompute what eq. 13 needs
+int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, float* dv_dev, const float2* F_reuse = nullptr)
 {
     if (p->normalise && (p->ix_begin != 0 || p->ix_end != p->gd.nx)) return DM_ERR_UNSUPPORTED;   // before any launch
     int rps = 1;
@@ -306,12 +317,18 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     stage_end(p, 0);
     const double *area_total = nullptr, *sdot = nullptr;
     if (p->normalise) {
-        // eq. 13's second term needs |Lambda| and sum_k Re(conj(G) F): one raw forward of these vertices and a dot product
+        // eq. 13's second term needs |Lambda| and sum_k Re(conj(G) F): the caller's spectrum u = F/|Lambda| of these vertices
+        // (then the dot product is taken with u), or one raw forward of these vertices
         const long long nk = (long long)n_k_of(p);
-        if (!p->spec3 && cudaMalloc(&p->spec3, (size_t)nk * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
         if (!p->dot_part && cudaMalloc(&p->dot_part, (DM_DOT_BLOCKS + 1) * sizeof(double)) != cudaSuccess) return DM_ERR_ALLOC;
-        if ((rc = run_forward_raw(p, vertices_dev, (float*)p->spec3))) return rc;
-        dm_k_dot_partial<<<DM_DOT_BLOCKS, 256, 0, p->stream>>>((const float2*)G_dev, p->spec3, nk, p->dot_part);
+        const float2* Fdot = F_reuse;
+        if (!Fdot) {
+            if (!p->spec3 && cudaMalloc(&p->spec3, (size_t)nk * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
+            p->F_valid = false;
+            if ((rc = run_forward_raw(p, vertices_dev, (float*)p->spec3))) return rc;
+            Fdot = p->spec3;
+        }
+        dm_k_dot_partial<<<DM_DOT_BLOCKS, 256, 0, p->stream>>>((const float2*)G_dev, Fdot, nk, p->dot_part);
         if ((rc = check_launch(p))) return rc;
         dm_k_dot_final<<<1, DM_DOT_BLOCKS, 0, p->stream>>>(p->dot_part, p->dot_part + DM_DOT_BLOCKS);
         if ((rc = check_launch(p))) return rc;
@@ -321,7 +338,7 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     stage_begin(p, 3);
     dm_k_corner_grads<<<(p->n_faces + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode,
                                                                        n_split, p->part, (const float2*)G_dev,
-                                                                       p->ix_begin == 0 ? 1 : 0, area_total, sdot, p->gd.face_w,
+                                                                       p->ix_begin == 0 ? 1 : 0, area_total, sdot, F_reuse != nullptr ? 1 : 0, p->gd.face_w,
                                                                        p->corner);
     rc = check_launch(p);
     if (rc) return rc;
@@ -477,7 +494,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
         // (up to 48 CTAs per SM slot), within 64 M floats of partial sums
         {
             const long long tri_blocks = ((long long)n_faces + 127) / 128;
-            long long m = ((long long)p->n_sm * 48 + tri_blocks - 1) / tri_blocks;
+            long long m = ((long long)p->n_sm * DM_BWD_SPLIT_TARGET + tri_blocks - 1) / tri_blocks;
             m = std::min<long long>(m, (64LL << 20) / ((long long)DM_BWD_NSUM * n_faces));
             p->n_split_max = (int)std::max<long long>(64, std::min<long long>(m, 4096));
             // the fast kernel's queue entries hold a 15-bit row index inside the split
@@ -501,7 +518,10 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
             const long long kblocks = ((long long)p->gd.nx * n_yruns * p->gd.nzh + DM_FAST_THREADS - 1) / DM_FAST_THREADS;
             const long long slots = (long long)p->n_sm * 4;
             long long want = (6 * slots + kblocks - 1) / kblocks;
-            want = std::min<long long>(want, std::max<long long>(1, n_faces / 384));   // at least one tile of strip records per chunk
+            // a chunk costs two flush records and one row of partial spectra: at least DM_FAST_MIN_CHUNK faces each.  Large
+            // meshes fill the machine with few chunks of whole tiles; a small mesh on a small grid (an
+            // 80-triangle sphere; :261: 10 000 such steps) needs the short chunks to reach every SM
+            want = std::min<long long>(want, std::max<long long>(1, n_faces / DM_FAST_MIN_CHUNK));
             want = std::max<long long>(1, std::min<long long>(want, 64));
             DmStripRecords sr;
             try { sr = dm_build_strips(faces_h.data(), n_faces, n_vertices, (int)want); } catch (...) { rc = DM_ERR_ALLOC; break; }
@@ -566,12 +586,14 @@ int dm_plan_set_slab(dm_plan* p, int32_t ix_begin, int32_t ix_end)
     if (!p || ix_begin < 0 || ix_end > p->gd.nx || ix_begin >= ix_end) return DM_ERR_INVALID_ARG;
     p->ix_begin = ix_begin;
     p->ix_end = ix_end;
+    p->F_valid = false;
     return DM_OK;
 }
 
 int dm_plan_set_face_weights(dm_plan* p, const float* weights_dev)
 {
     if (!p) return DM_ERR_INVALID_ARG;
+    p->F_valid = false;
     if (!weights_dev) {
         p->gd.face_w = nullptr;
         p->weights_robust = false;
@@ -623,6 +645,7 @@ int dm_plan_set_face_weights(dm_plan* p, const float* weights_dev)
 int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
 {
     if (!p) return DM_ERR_INVALID_ARG;
+    p->F_valid = false;
     if (!psf_cov_host) {
         p->band_on = false;
         p->gd.band_lim = INFINITY;
@@ -718,7 +741,12 @@ int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
 int dm_plan_set_option(dm_plan* p, int option, double value)
 {
     if (!p) return DM_ERR_INVALID_ARG;
+    if (option != DM_OPT_REUSE_SPECTRUM) p->F_valid = false;
     switch (option) {
+        case DM_OPT_REUSE_SPECTRUM:
+            if (value != 0.0 && value != 1.0) return DM_ERR_INVALID_ARG;
+            p->reuse_F = value == 1.0;
+            return DM_OK;
         case DM_OPT_FORWARD_PATH:
             if (value != 0.0 && value != 1.0) return DM_ERR_INVALID_ARG;
             p->fwd_path = (int)value;
@@ -747,6 +775,7 @@ int dm_plan_set_option(dm_plan* p, int option, double value)
 int dm_mesh_ft_forward(dm_plan* p, const float* vertices_dev, float* F_dev)
 {
     if (!p || !vertices_dev || !F_dev) return DM_ERR_INVALID_ARG;
+    p->F_valid = false;   // the plan's total area / volume now belongs to these vertices
     stage_reset(p);
     stage_begin(p, 0);
     const int rc = run_forward(p, vertices_dev, F_dev);
@@ -760,6 +789,15 @@ int dm_mesh_ft_backward(dm_plan* p, const float* vertices_dev, const float* dL_d
     stage_reset(p);
     stage_begin(p, 0);
     return run_backward(p, vertices_dev, dL_dF_dev, dL_dvertices_dev);
+}
+
+int dm_mesh_ft_backward_with_spectrum(dm_plan* p, const float* vertices_dev, const float* dL_dF_dev, const float* F_dev,
+                                      float* dL_dvertices_dev)
+{
+    if (!p || !vertices_dev || !dL_dF_dev || !F_dev || !dL_dvertices_dev) return DM_ERR_INVALID_ARG;
+    stage_reset(p);
+    stage_begin(p, 0);
+    return run_backward(p, vertices_dev, dL_dF_dev, dL_dvertices_dev, p->normalise ? (const float2*)F_dev : nullptr);
 }
 
 int dm_spectrum_to_image(dm_plan* p, const float* F_dev, const float* psf_cov_host, float* image_dev)
@@ -793,11 +831,15 @@ int dm_render(dm_plan* p, const float* vertices_dev, const float* psf_cov_host, 
     if (rc) return rc;
     if ((rc = ensure_fft(p))) return rc;
     stage_reset(p);
+    if (!p->spec3 && cudaMalloc(&p->spec3, n_k_of(p) * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
+    p->F_valid = false;
     stage_begin(p, 0);
-    rc = run_forward(p, vertices_dev, (float*)p->spec2);
+    rc = run_forward(p, vertices_dev, (float*)p->spec3);   // F stays in the plan for dm_render_backward (DM_OPT_REUSE_SPECTRUM)
     stage_end(p, 0);
     if (rc) return rc;
-    return run_spectrum_to_image(p, (const float*)p->spec2, psf, image_dev);
+    rc = run_spectrum_to_image(p, (const float*)p->spec3, psf, image_dev);
+    p->F_valid = rc == DM_OK;
+    return rc;
 }
 
 int dm_render_backward(dm_plan* p, const float* vertices_dev, const float* psf_cov_host, const float* dL_dimage_dev,
@@ -809,6 +851,8 @@ int dm_render_backward(dm_plan* p, const float* vertices_dev, const float* psf_c
     int rc = make_psf(p, psf_cov_host, &psf);
     if (rc) return rc;
     if ((rc = ensure_fft(p))) return rc;
+    const bool reuse = p->reuse_F && (dL_dpsf_cov_host || p->normalise);
+    if (reuse && !p->F_valid) return DM_ERR_INVALID_ARG;   // no dm_render spectrum to reuse (or something changed since)
     if (dL_dpsf_cov_host) {
         const size_t nk = n_k_of(p);
         if (!p->spec3 && cudaMalloc(&p->spec3, nk * sizeof(float2)) != cudaSuccess) return DM_ERR_ALLOC;
@@ -819,10 +863,14 @@ int dm_render_backward(dm_plan* p, const float* vertices_dev, const float* psf_c
     rc = run_image_to_cotangent(p, dL_dimage_dev, psf, (float*)p->spec2);   // leaves R = rfft3(dL/dimage) in p->spec
     if (rc) return rc;
     stage_begin(p, 0);
-    rc = run_backward(p, vertices_dev, (const float*)p->spec2, dL_dvertices_dev);
+    rc = run_backward(p, vertices_dev, (const float*)p->spec2, dL_dvertices_dev, reuse ? p->spec3 : nullptr);
     if (rc || !dL_dpsf_cov_host) return rc;
-    // PSF-parameter gradient: needs the forward spectrum F of these vertices (recomputed: one forward mesh FT)
-    if ((rc = run_forward(p, vertices_dev, (float*)p->spec3))) return rc;
+    // PSF-parameter gradient: needs the forward spectrum F of these vertices -- the one dm_render left in the plan
+    // (DM_OPT_REUSE_SPECTRUM), else recomputed (one forward mesh FT)
+    if (!reuse) {
+        p->F_valid = false;
+        if ((rc = run_forward(p, vertices_dev, (float*)p->spec3))) return rc;
+    }
     dm_k_psf_grad_partial<<<DM_PSFG_BLOCKS, 256, 0, p->stream>>>(p->spec, p->spec3, p->gd, psf, p->psfg_part);
     if ((rc = check_launch(p))) return rc;
     dm_k_psf_grad_final<<<1, DM_PSFG_BLOCKS, 0, p->stream>>>(p->psfg_part, p->psfg_out);

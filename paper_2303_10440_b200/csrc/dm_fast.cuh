@@ -38,6 +38,9 @@ static_assert(DM_STRIP_UNROLL == 6, "the strip loop is unrolled by 6 (window per
 #define DM_FORCE_OUTLIER_RATIO2 6.25f //   h_T^2 > 6.25 h_rms^2
 #define DM_LOWK_RADIUS 0.5f         // |k| h_max below which a frequency is "low" (all gaps small for all triangles)
 #define DM_LOWK_BOX 24              // low-k kernel covers |n_a| <= DM_LOWK_BOX
+#ifndef DM_FAST_MIN_CHUNK
+#define DM_FAST_MIN_CHUNK 48        // fewest faces per strip chunk (host policy of dm_plan_create)
+#endif
 
 // strip record = 3 x float4 (48 B):
 //   r0 = (u_ret.xyz [uint32 bit patterns], rho_ret.re)     retiring vertex: fixed-point position, y-rotation
@@ -323,68 +326,73 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
 }
 
 // ---- A4 at low |k|: every pair through the robust branches; one CTA per frequency, threads stride over the records ----
-// grid = the (2B+1)^2 (B+1) frequencies of the low-k box (most CTAs leave at once); writes F directly.  The block sum is
-// taken in a fixed order (lane tree, then the warps in order): deterministic.
+// The CTAs stride over the (2 bx + 1)(2 by + 1)(bz + 1) candidate frequencies |n_x| <= bx, |n_y| <= by, n_z <= bz (the low-k
+// box clipped to the grid); a candidate that is not "low" costs one test.  Writes F directly.  The block sum is taken in
+// a fixed order (lane tree, then the warps in order): deterministic.
 #define DM_LOWK_THREADS 256
 template <int MODE>
 __global__ void __launch_bounds__(DM_LOWK_THREADS)
 dm_k_forward_lowk(const float4* __restrict__ rec, const int32_t* __restrict__ chunk_off, int n_chunks, DmGridDev grid,
-                  int ix_begin, int ix_end, const unsigned int* __restrict__ hmax2_bits, float2* __restrict__ F)
+                  int ix_begin, int ix_end, int bx, int by, int bz, const unsigned int* __restrict__ hmax2_bits,
+                  float2* __restrict__ F)
 {
     __shared__ float wsum[2][DM_LOWK_THREADS / 32];
-    const int B = DM_LOWK_BOX, W = 2 * B + 1;
-    const int fi = blockIdx.x, lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-    if (fi >= W * W * (B + 1)) return;
-    const int nz = fi % (B + 1), nys = (fi / (B + 1)) % W - B, nx = fi / ((B + 1) * W) - B;
-    if (nz > grid.nz / 2 || nys < -(grid.ny / 2) || nys > (grid.ny - 1) / 2 || nx < -(grid.nx / 2) || nx > (grid.nx - 1) / 2) return;
-    const int ix = nx < 0 ? nx + grid.nx : nx, iy = nys < 0 ? nys + grid.ny : nys;
-    if (ix < ix_begin || ix >= ix_end) return;
-    if (!dm_k_is_low(grid, nx, nys, nz, __uint_as_float(*hmax2_bits)) || !dm_in_band(grid, nx, nys, nz)) return;
-    const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * nys, kz = grid.kstep[2] * nz;
-    float are = 0.f, aim = 0.f;
-    for (int c = 0; c < n_chunks; ++c) {
-        const int b = chunk_off[c], e = chunk_off[c + 1];
-        for (int i = b + 1 + (int)threadIdx.x; i < e; i += DM_LOWK_THREADS) {   // record b closes no triangle
-            const float4 r2 = rec[3 * (size_t)i + 2];
-            const bool valid = (MODE == 1) ? (r2.x != 0.f) : (r2.x != 0.f || r2.y != 0.f || r2.z != 0.f);
-            if (!valid) continue;
-            const float4 r0 = rec[3 * (size_t)i], r1 = rec[3 * (size_t)i + 1], q1 = rec[3 * (size_t)i - 2];
-            const float p = fmaf(kx, q1.y, fmaf(ky, q1.z, kz * q1.w));
-            const float q = p + fmaf(kx, r1.y, fmaf(ky, r1.z, kz * r1.w));
-            cf psi, d1, d2;
-            dm_psi_robust<false>(p, q, psi, d1, d2);
-            const cf E = dm_expmi_turns(dm_phase_turns(nx, nys, nz, __float_as_uint(r0.x), __float_as_uint(r0.y),
-                                                       __float_as_uint(r0.z)));
-            const float sc = (MODE == 1) ? r2.x : fmaf(kx, r2.x, fmaf(ky, r2.y, kz * r2.z));
-            const cf g = cmul(E, psi);
-            are = fmaf(sc, g.re, are);
-            aim = fmaf(sc, g.im, aim);
+    const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+    const int Wy = 2 * by + 1, n_cand = (2 * bx + 1) * Wy * (bz + 1);
+    const float hmax2 = __uint_as_float(*hmax2_bits);
+    for (int fi = blockIdx.x; fi < n_cand; fi += gridDim.x) {
+        const int nz = fi % (bz + 1), nys = (fi / (bz + 1)) % Wy - by, nx = fi / ((bz + 1) * Wy) - bx;
+        if (nz > grid.nz / 2 || nys < -(grid.ny / 2) || nys > (grid.ny - 1) / 2 || nx < -(grid.nx / 2) || nx > (grid.nx - 1) / 2) continue;
+        const int ix = nx < 0 ? nx + grid.nx : nx, iy = nys < 0 ? nys + grid.ny : nys;
+        if (ix < ix_begin || ix >= ix_end) continue;
+        if (!dm_k_is_low(grid, nx, nys, nz, hmax2) || !dm_in_band(grid, nx, nys, nz)) continue;
+        const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * nys, kz = grid.kstep[2] * nz;
+        float are = 0.f, aim = 0.f;
+        for (int c = 0; c < n_chunks; ++c) {
+            const int b = chunk_off[c], e = chunk_off[c + 1];
+            for (int i = b + 1 + (int)threadIdx.x; i < e; i += DM_LOWK_THREADS) {   // record b closes no triangle
+                const float4 r2 = rec[3 * (size_t)i + 2];
+                const bool valid = (MODE == 1) ? (r2.x != 0.f) : (r2.x != 0.f || r2.y != 0.f || r2.z != 0.f);
+                if (!valid) continue;
+                const float4 r0 = rec[3 * (size_t)i], r1 = rec[3 * (size_t)i + 1], q1 = rec[3 * (size_t)i - 2];
+                const float p = fmaf(kx, q1.y, fmaf(ky, q1.z, kz * q1.w));
+                const float q = p + fmaf(kx, r1.y, fmaf(ky, r1.z, kz * r1.w));
+                cf psi, d1, d2;
+                dm_psi_robust<false>(p, q, psi, d1, d2);
+                const cf E = dm_expmi_turns(dm_phase_turns(nx, nys, nz, __float_as_uint(r0.x), __float_as_uint(r0.y),
+                                                           __float_as_uint(r0.z)));
+                const float sc = (MODE == 1) ? r2.x : fmaf(kx, r2.x, fmaf(ky, r2.y, kz * r2.z));
+                const cf g = cmul(E, psi);
+                are = fmaf(sc, g.re, are);
+                aim = fmaf(sc, g.im, aim);
+            }
         }
-    }
-    for (int o = 16; o > 0; o >>= 1) {
-        are += __shfl_xor_sync(0xffffffffu, are, o);
-        aim += __shfl_xor_sync(0xffffffffu, aim, o);
-    }
-    if (lane == 0) {
-        wsum[0][wrp] = are;
-        wsum[1][wrp] = aim;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        are = 0.f, aim = 0.f;
+        for (int o = 16; o > 0; o >>= 1) {
+            are += __shfl_xor_sync(0xffffffffu, are, o);
+            aim += __shfl_xor_sync(0xffffffffu, aim, o);
+        }
+        __syncthreads();   // the previous candidate's sums have been read
+        if (lane == 0) {
+            wsum[0][wrp] = are;
+            wsum[1][wrp] = aim;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            are = 0.f, aim = 0.f;
 #pragma unroll
-        for (int w = 0; w < DM_LOWK_THREADS / 32; ++w) {
-            are += wsum[0][w];
-            aim += wsum[1][w];
+            for (int w = 0; w < DM_LOWK_THREADS / 32; ++w) {
+                are += wsum[0][w];
+                aim += wsum[1][w];
+            }
+            if (MODE == 0) {
+                const float k2 = kx * kx + ky * ky + kz * kz;
+                const float ik2 = (k2 > 0.f) ? 1.0f / k2 : 0.f;
+                const float t = are;
+                are = -aim * ik2;
+                aim = t * ik2;
+            }
+            F[((size_t)ix * grid.ny + iy) * grid.nzh + nz] = make_float2(are, aim);
         }
-        if (MODE == 0) {
-            const float k2 = kx * kx + ky * ky + kz * kz;
-            const float ik2 = (k2 > 0.f) ? 1.0f / k2 : 0.f;
-            const float t = are;
-            are = -aim * ik2;
-            aim = t * ik2;
-        }
-        F[((size_t)ix * grid.ny + iy) * grid.nzh + nz] = make_float2(are, aim);
     }
 }
 

@@ -283,7 +283,7 @@ dm_k_backward_robust(const float4* __restrict__ rec, int n_faces, DmGridDev grid
 __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int32_t* __restrict__ faces, int n_faces,
                                   int mode, int n_split, const float* __restrict__ part,
                                   const float2* __restrict__ G, int has_dc, const double* __restrict__ area_total,
-                                  const double* __restrict__ sdot, const float* __restrict__ face_w,
+                                  const double* __restrict__ sdot, int sdot_of_u, const float* __restrict__ face_w,
                                   float* __restrict__ corner)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -301,7 +301,8 @@ __global__ void dm_k_corner_grads(const float* __restrict__ vertices, const int3
         const double inv = 1.0 / *area_total;
 #pragma unroll
         for (int j = 0; j < DM_BWD_NSUM; ++j) s[j] = (float)((double)s[j] * inv);
-        s[0] = (float)((double)s[0] - 0.5 * (*sdot) * inv * inv);
+        // (*sdot = sum_k Re(conj(G) F) with the raw F, or with u = F/|Lambda| itself when sdot_of_u is set)
+        s[0] = (float)((double)s[0] - 0.5 * (*sdot) * (sdot_of_u ? inv : inv * inv));
     }
     const int idx[3] = {faces[3 * t], faces[3 * t + 1], faces[3 * t + 2]};
     float v[3][3];

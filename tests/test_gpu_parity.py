@@ -479,3 +479,82 @@ def test_stretched_meshes_and_outlier_faces(dm, mode):
         dref = oracle.mesh_ft_backward_grid(v, f, n, spacing, mode, G.astype(np.complex128))
         assert _rel_l2(dv, dref) <= GRAD_TOL, (len(f), _rel_l2(dv, dref))
         plan.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_tall_grid_fast_kernels(dm, mode):
+    """A grid much longer along z than one super-segment of the backward kernel (N_z/2+1 = 321 > 288: two super-segments
+    with their own exact start phases, 32-frequency seed spacing) -- the paper's image sizes go up to 2048^3
+    (PAPER.md:59).  Both passes must stay on the fast kernels and match the oracle on the full grid."""
+    w = build_workload(1, grid_override=(16, 16, 640))
+    G = spectrum_cotangent(w)
+    plan = _plan(dm, w, mode)
+    vd = _dev(w.vertices)
+    F = plan.mesh_ft_forward(vd).cpu().numpy()
+    ref = oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, mode)
+    assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0])
+    dv = plan.mesh_ft_backward(vd, _dev(G)).cpu().numpy()
+    assert plan.paths_used() == (0, 0)
+    dref = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, mode, G.astype(np.complex128))
+    assert _rel_l2(dv, dref) <= GRAD_TOL
+    # the same under a narrow band that cuts the rows short at different z
+    cov = (np.array([2.0, 2.0, 3.0]) * np.array(w.spacing)) ** 2
+    plan.set_narrow_band([cov[0], cov[1], cov[2], 0.0, 0.0, 0.0], 0.01)
+    dvb = plan.mesh_ft_backward(vd, _dev(G)).cpu().numpy()
+    Fb = plan.mesh_ft_forward(vd).cpu().numpy()
+    inb = Fb != 0
+    inb[0, 0, 0] = True
+    Gb = np.where(inb, G, 0).astype(np.complex128)
+    drefb = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, mode, Gb)
+    assert _rel_l2(dvb, drefb) <= GRAD_TOL
+    plan.close()
+
+
+def test_reuse_of_the_render_spectrum(dm):
+    """DM_OPT_REUSE_SPECTRUM / dm_mesh_ft_backward_with_spectrum (shape and PSF are fitted in one
+    loop): the PSF gradient and eq. 13's extra term computed from the spectrum the forward call already produced must
+    equal the recomputing path, use fewer launches, and refuse to run when the plan holds no such spectrum."""
+    import torch
+    w = build_workload(2, subdiv_override=2, grid_override=(24, 20, 16))
+    cov = w.psf_cov.astype(np.float64)
+    y = torch.as_tensor(np.random.default_rng(5).standard_normal(w.n).astype(np.float32), device="cuda")
+    for mode, normalised in ((0, False), (1, False), (1, True)):
+        plan, vd = _plan(dm, w, mode), _dev(w.vertices)
+        if normalised:
+            plan.set_option(dm.DM_OPT_AREA_NORMALISED, 1)
+        plan.render(vd, cov)
+        n0 = plan.launch_count()
+        dv_a, dc_a = plan.render_backward(vd, cov, y, with_psf_grad=True)
+        n_recompute = plan.launch_count() - n0
+        dv_a = dv_a.clone()
+        plan.set_option(dm.DM_OPT_REUSE_SPECTRUM, 1)
+        with pytest.raises(dm.DeltamicError):          # the option change invalidated nothing, but the recompute did
+            plan.render_backward(vd, cov, y, with_psf_grad=True)
+        plan.render(vd, cov)
+        n0 = plan.launch_count()
+        dv_b, dc_b = plan.render_backward(vd, cov, y, with_psf_grad=True)
+        n_reuse = plan.launch_count() - n0
+        assert n_reuse < n_recompute
+        assert torch.equal(dv_a, dv_b) or _rel_l2(dv_b.cpu().numpy(), dv_a.cpu().numpy()) <= 1e-6
+        assert np.allclose(dc_a, dc_b, rtol=1e-5, atol=1e-6 * np.abs(dc_a).max())
+        dv_c = plan.render_backward(vd, cov, y)        # may be called again: the spectrum stays valid
+        assert _rel_l2(dv_c.cpu().numpy(), dv_a.cpu().numpy()) <= 1e-6
+        plan.mesh_ft_forward(vd)                       # any other forward call invalidates it
+        if normalised:
+            with pytest.raises(dm.DeltamicError):
+                plan.render_backward(vd, cov, y)
+        plan.close()
+    # the mesh-FT pair of calls with the area-normalised density
+    plan, vd = _plan(dm, w, 1), _dev(w.vertices)
+    plan.set_option(dm.DM_OPT_AREA_NORMALISED, 1)
+    G = _dev(spectrum_cotangent(w))
+    u = plan.mesh_ft_forward(vd)
+    n0 = plan.launch_count()
+    d1 = plan.mesh_ft_backward(vd, G).clone()
+    n1 = plan.launch_count() - n0
+    u = plan.mesh_ft_forward(vd)
+    n0 = plan.launch_count()
+    d2 = plan.mesh_ft_backward(vd, G, spectrum=u)
+    n2 = plan.launch_count() - n0
+    assert n2 < n1 and _rel_l2(d2.cpu().numpy(), d1.cpu().numpy()) <= 1e-6
+    plan.close()
