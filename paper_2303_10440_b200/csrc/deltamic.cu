@@ -336,8 +336,14 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
         sdot = p->dot_part + DM_DOT_BLOCKS;
     }
     stage_begin(p, 3);
+    int n_split_left = n_split;
+    if (n_split > 4) {   // many splits (small meshes): sum them with 13x the threads first
+        dm_k_sum_splits<<<dim3((p->n_faces + 127) / 128, DM_BWD_NSUM), 128, 0, p->stream>>>(p->part, p->n_faces, n_split);
+        if ((rc = check_launch(p))) return rc;
+        n_split_left = 1;
+    }
     dm_k_corner_grads<<<(p->n_faces + 127) / 128, 128, 0, p->stream>>>(vertices_dev, p->faces, p->n_faces, p->mode,
-                                                                       n_split, p->part, (const float2*)G_dev,
+                                                                       n_split_left, p->part, (const float2*)G_dev,
                                                                        p->ix_begin == 0 ? 1 : 0, area_total, sdot, F_reuse != nullptr ? 1 : 0, p->gd.face_w,
                                                                        p->corner);
     rc = check_launch(p);

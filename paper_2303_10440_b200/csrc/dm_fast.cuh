@@ -39,7 +39,7 @@ static_assert(DM_STRIP_UNROLL == 6, "the strip loop is unrolled by 6 (window per
 #define DM_LOWK_RADIUS 0.5f         // |k| h_max below which a frequency is "low" (all gaps small for all triangles)
 #define DM_LOWK_BOX 24              // low-k kernel covers |n_a| <= DM_LOWK_BOX
 #ifndef DM_FAST_MIN_CHUNK
-#define DM_FAST_MIN_CHUNK 48        // fewest faces per strip chunk (host policy of dm_plan_create)
+#define DM_FAST_MIN_CHUNK 16        // fewest faces per strip chunk (host policy of dm_plan_create)
 #endif
 
 // strip record = 3 x float4 (48 B):

@@ -275,6 +275,20 @@ dm_k_backward_robust(const float4* __restrict__ rec, int n_faces, DmGridDev grid
     }
 }
 
+// ---- A6 (end): sum the k-splits of every (sum, triangle) in fixed order into split 0's slot ---------------------------
+// grid = (ceil(n_faces/128), 13): coalesced over triangles; a small mesh has hundreds of splits, which one thread per
+// triangle would walk alone.
+__global__ void __launch_bounds__(128)
+dm_k_sum_splits(float* __restrict__ part, int n_faces, int n_split)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_faces) return;
+    const size_t o = (size_t)blockIdx.y * n_faces + t;
+    float s = 0.f;
+    for (int sp = 0; sp < n_split; ++sp) s += part[(size_t)sp * DM_BWD_NSUM * n_faces + o];
+    part[o] = s;
+}
+
 // ---- A6 (end): sum the splits in fixed order and form the per-corner gradients ------------------------------------
 //   surface (eq. 10):  grad_p = -w_p S0 + |m_T| V_p,     w_p = e_p x N_T, e_p = v_{p-} - v_{p+}
 //   volume  (product rule, d(k.m_T)/dv_p = k x e_p):  grad_p = Q x e_p + V_p,  plus the k = 0 row
