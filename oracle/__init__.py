@@ -8,7 +8,8 @@ image-formation reference (PSF multiply + inverse rFFT).
 Parity status: every function here is pinned by `-m "not gpu"` tests (tests/test_oracle_*.py) except
 the behaviour of an inverse real FFT on a half spectrum that is not exactly Hermitian on its
 self-conjugate planes (reading R13), where the oracle *defines* the semantics as numpy/pocketfft's
-irfftn -- "parity unpinned" for that one convention.
+irfftn -- "parity unpinned" for that one convention.  oracle/shape_step.py (the shape-optimisation step of PAPER.md:244-249) is
+pinned by tests/test_oracle_shape.py.
 """
 from .mesh_ft import (  # noqa: F401
     frequency_grid,
@@ -27,3 +28,5 @@ from .mesh_ft import (  # noqa: F401
 )
 from .render import (psf_shift_spectrum, render, render_backward, render_backward_psf, spectrum_to_image,  # noqa: F401
                      image_to_spectrum_cotangent)
+from .shape_step import (AdamUniformState, ShapeParams, ShapeState, adam_uniform_step, connectivity_laplacian,  # noqa: F401
+                         phi1, phi1_grad, precondition, shape_step)
