@@ -183,6 +183,46 @@ int dm_plan_paths_used(const dm_plan* plan, int32_t paths[2]);
 
 void dm_plan_destroy(dm_plan* plan);
 
+/* ---- Shape-optimisation step (section 5.1.3, eq. 17; readings R26-R28 of DESIGN.md) ------------------
+ *   Phi_1 = sum_voxels (u - m)^2 m                      u = dm_render(vertices), m = the target image
+ *   g     = dPhi_1/dvertices                            through dm_render_backward
+ *   g~    = (I + lambda L)^-2 g                         L = D - A, the connectivity Laplacian of the mesh's vertex graph;
+ *                                                       two conjugate-gradient solves with I + lambda L on the device
+ *                                                       (the paper uses a sparse Cholesky factorisation), fp64
+ *   vertices <- AdamUniform(vertices, g~)               m_t = b1 m + (1-b1) g~,  s_t = b2 s + (1-b2) max_i g~_i^2,
+ *                                                       v -= lr (m_t/(1-b1^t)) / (sqrt(s_t/(1-b2^t)) + eps)
+ * The state owns the vertex graph, the optimiser moments (zero at creation) and all scratch; it belongs to ONE plan
+ * (and must be destroyed before it).  The step honours the plan's narrow band (the shape step runs on
+ * the narrow band), slab must be the whole grid.  Everything is queued on the plan's stream; nothing synchronises
+ * unless loss_host is given. */
+typedef struct dm_shape_state dm_shape_state; /* opaque */
+
+typedef struct dm_shape_params {
+    float   lr;          /* eta of eq. 17 (default 1e-3)                                              */
+    float   lambda;      /* diffusion weight (default 50)                               */
+    float   beta1;       /* first-moment decay (default 0.9)                                          */
+    float   beta2;       /* second-moment decay (default 0.999)                                       */
+    float   eps;         /* default 1e-8                                                              */
+    float   cg_tol;      /* a solve stops when |r| <= cg_tol |b| on every column (default 1e-7)       */
+    int32_t cg_max_iter; /* launches are queued for this many iterations per solve (default 400)      */
+} dm_shape_params;
+
+int dm_shape_params_default(dm_shape_params* out);
+
+/* params = NULL takes the defaults.  Synchronises the stream (it uploads the vertex graph). */
+int dm_shape_state_create(dm_plan* plan, const dm_shape_params* params, dm_shape_state** out);
+
+/* out = (I + lambda L)^-2 g for a float32 [n_vertices*3] field g (both DEVICE pointers; they may be the same). */
+int dm_shape_precondition(dm_plan* plan, dm_shape_state* state, const float* g_dev, float* out_dev);
+
+/* One step.  vertices_dev float32 [n_vertices*3] is updated IN PLACE; target_dev float32 [n_x*n_y*n_z] is the image m;
+ * psf_cov_host as in dm_render.  loss_host = NULL, or a HOST double that receives Phi_1 of the vertices BEFORE the
+ * step (the call then synchronises the stream). */
+int dm_shape_step(dm_plan* plan, dm_shape_state* state, float* vertices_dev, const float* target_dev,
+                  const float* psf_cov_host, double* loss_host);
+
+void dm_shape_state_destroy(dm_shape_state* state);
+
 const char* dm_error_string(int code);
 
 /* Library version as major*10000 + minor*100 + patch. */

@@ -16,11 +16,13 @@ from ._binding import (  # noqa: F401
     DM_VOLUME,
     DeltamicError,
     Plan,
+    ShapeParams,
+    ShapeState,
     exported_symbols,
     library_path,
     load_library,
     version,
 )
 
-__all__ = ["Plan", "DM_VOLUME", "DM_SURFACE", "DeltamicError", "load_library", "library_path", "exported_symbols",
+__all__ = ["Plan", "ShapeState", "ShapeParams", "DM_VOLUME", "DM_SURFACE", "DeltamicError", "load_library", "library_path", "exported_symbols",
            "version"]

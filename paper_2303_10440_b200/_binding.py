@@ -16,6 +16,7 @@ _SYMBOLS = (
     "dm_plan_create", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_mesh_ft_backward_with_spectrum", "dm_render",
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
     "dm_plan_launch_count", "dm_plan_paths_used", "dm_plan_destroy", "dm_error_string", "dm_version",
+    "dm_shape_params_default", "dm_shape_state_create", "dm_shape_precondition", "dm_shape_step", "dm_shape_state_destroy",
 )
 
 
@@ -23,6 +24,12 @@ class DeltamicError(RuntimeError):
     def __init__(self, code: int, what: str):
         super().__init__(f"{what} failed: {code} ({_err(code)})")
         self.code = code
+
+
+class ShapeParams(ctypes.Structure):
+    """dm_shape_params (include/deltamic.h)."""
+    _fields_ = [("lr", ctypes.c_float), ("lambda_", ctypes.c_float), ("beta1", ctypes.c_float), ("beta2", ctypes.c_float),
+                ("eps", ctypes.c_float), ("cg_tol", ctypes.c_float), ("cg_max_iter", ctypes.c_int32)]
 
 
 class _Grid(ctypes.Structure):
@@ -73,9 +80,15 @@ def load_library():
     lib.dm_error_string.argtypes = [ctypes.c_int]
     lib.dm_error_string.restype = ctypes.c_char_p
     lib.dm_version.restype = ctypes.c_int
+    lib.dm_shape_params_default.argtypes = [ctypes.POINTER(ShapeParams)]
+    lib.dm_shape_state_create.argtypes = [vp, ctypes.POINTER(ShapeParams), ctypes.POINTER(vp)]
+    lib.dm_shape_precondition.argtypes = [vp, vp, fp, fp]
+    lib.dm_shape_step.argtypes = [vp, vp, fp, fp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]
+    lib.dm_shape_state_destroy.argtypes = [vp]
+    lib.dm_shape_state_destroy.restype = None
     for name in _SYMBOLS:
         fn = getattr(lib, name)
-        if name not in ("dm_plan_launch_count", "dm_plan_destroy", "dm_error_string"):
+        if name not in ("dm_plan_launch_count", "dm_plan_destroy", "dm_error_string", "dm_shape_state_destroy"):
             fn.restype = ctypes.c_int
     _lib = lib
     return lib
@@ -254,9 +267,63 @@ class Plan:
         _check(self._lib.dm_plan_paths_used(self._h, out), "dm_plan_paths_used")
         return int(out[0]), int(out[1])
 
+    def shape_state(self, **params):
+        """A ShapeState (dm_shape_state) of this plan; keyword arguments override dm_shape_params' defaults
+        (lr, lambda_, beta1, beta2, eps, cg_tol, cg_max_iter)."""
+        return ShapeState(self, **params)
+
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
             self._lib.dm_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class ShapeState:
+    """Optimiser state of the shape-optimisation step (dm_shape_state).  Argument marshalling only."""
+
+    def __init__(self, plan: Plan, **params):
+        self._plan = plan
+        self._lib = plan._lib
+        prm = ShapeParams()
+        _check(self._lib.dm_shape_params_default(ctypes.byref(prm)), "dm_shape_params_default")
+        for k, v in params.items():
+            if not hasattr(prm, k):
+                raise TypeError(f"unknown shape parameter {k}")
+            setattr(prm, k, v)
+        self.params = prm
+        h = ctypes.c_void_p()
+        _check(self._lib.dm_shape_state_create(plan._h, ctypes.byref(prm), ctypes.byref(h)), "dm_shape_state_create")
+        self._h = h
+
+    def precondition(self, g, out=None):
+        """(I + lambda L)^-2 g for a float32 CUDA tensor [n_vertices, 3]."""
+        p = self._plan
+        gg = p._f32(g, p.n_vertices * 3, "g")
+        if out is None:
+            out = p._torch.empty((p.n_vertices, 3), dtype=p._torch.float32, device=p.device)
+        o = p._f32(out, p.n_vertices * 3, "out")
+        _check(self._lib.dm_shape_precondition(p._h, self._h, gg.data_ptr(), o.data_ptr()), "dm_shape_precondition")
+        return out
+
+    def step(self, vertices, target, psf_cov, return_loss: bool = False):
+        """One step; ``vertices`` is updated in place.  With ``return_loss`` returns Phi_1 before the step (synchronises)."""
+        p = self._plan
+        v = p._vertices(vertices)
+        t = p._f32(target, p.n[0] * p.n[1] * p.n[2], "target")
+        loss = ctypes.c_double() if return_loss else None
+        _check(self._lib.dm_shape_step(p._h, self._h, v.data_ptr(), t.data_ptr(), _cov(psf_cov),
+                                       ctypes.byref(loss) if return_loss else None), "dm_shape_step")
+        return float(loss.value) if return_loss else None
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.dm_shape_state_destroy(self._h)
             self._h = ctypes.c_void_p()
 
     def __del__(self):  # pragma: no cover

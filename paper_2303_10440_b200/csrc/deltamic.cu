@@ -3,17 +3,20 @@
 #include <cuda_runtime.h>
 #include <cufft.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "../../include/deltamic.h"
 #include "dm_fast.cuh"
 #include "dm_bwd_fast.cuh"
 #include "dm_strips.h"
+#include "dm_shape.cuh"
 
 #define DM_VERSION 100
 #ifndef DM_BWD_SPLIT_TARGET
@@ -58,6 +61,7 @@ struct dm_plan {
     bool weights_robust = false;     // the weights are outside the regime the fast kernels are validated for (mixed
                                      // sign, or varying inside a connected component in volume mode): every pair goes
                                      // through the robust kernels
+    std::vector<int32_t> faces_host; // host copy of the faces (the shape-optimisation state builds the vertex graph from it)
     std::vector<int32_t> face_comp;  // host: connected component (shared vertices) of every face, built at create
     int last_fwd_path = -1, last_bwd_path = -1;   // 0 = fast, 1 = robust: what the last mesh-FT calls actually ran
     long long band_count = 0;        // stored frequencies inside the narrow band (whole grid)
@@ -495,6 +499,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
             for (int32_t t = 0; t < n_faces; ++t) p->face_comp[t] = find(faces_h[3 * (size_t)t]);
         } catch (...) { rc = DM_ERR_ALLOC; break; }
 
+        try { p->faces_host = faces_h; } catch (...) { rc = DM_ERR_ALLOC; break; }
         const size_t nk = n_k_of(p);
         // k-splits of the backward: a small mesh has few triangle blocks, so it needs many splits to fill the machine
         // (up to 48 CTAs per SM slot), within 64 M floats of partial sums
@@ -948,6 +953,212 @@ void dm_plan_destroy(dm_plan* p)
     if (p->ev_ok)
         for (int i = 0; i < 8; ++i) cudaEventDestroy(p->ev[i]);
     delete p;
+}
+
+}  // extern "C"
+
+// ---- shape-optimisation step (eq. 17) -------------------------------------------------------------------
+struct dm_shape_state {
+    dm_plan* plan = nullptr;
+    dm_shape_params prm;
+    int n_blocks = 0;                // ceil(n_vertices / DM_SH_THREADS)
+    int32_t *adj_off = nullptr, *adj_idx = nullptr;   // CSR of the distinct neighbours of every vertex (L = D - A)
+    double *cg_x = nullptr, *cg_y = nullptr, *cg_r = nullptr, *cg_p = nullptr, *cg_Ap = nullptr;
+    double *part_a = nullptr, *part_b = nullptr, *rr_next = nullptr;
+    DmCgScalars* cg_sc = nullptr;
+    double *mom = nullptr, *amax_part = nullptr, *s_next = nullptr;
+    DmAdamScalars* adam = nullptr;
+    float *image = nullptr, *cot = nullptr, *grad = nullptr;
+    double *loss_part = nullptr, *loss = nullptr;
+};
+
+namespace {
+
+// x = M^-1 b, M = I + lambda L, for the three columns of b ([n][3], fp32 or fp64), by conjugate gradients on the device
+template <typename TB>
+int shape_cg_solve(dm_plan* p, dm_shape_state* st, const TB* b_dev, double* x_dev)
+{
+    const int n = p->n_vertices, nb = st->n_blocks;
+    dm_k_cg_init<TB><<<nb, DM_SH_THREADS, 0, p->stream>>>(b_dev, n, x_dev, st->cg_r, st->cg_p, st->part_a);
+    dm_k_cg_init_final<<<1, DM_SH_THREADS, 0, p->stream>>>(st->part_a, nb, st->cg_sc);
+    int rc = check_launch(p, 2);
+    const double tol2 = (double)st->prm.cg_tol * (double)st->prm.cg_tol;
+    for (int it = 0; it < st->prm.cg_max_iter && rc == DM_OK; ++it) {
+        dm_k_cg_spmv<<<nb, DM_SH_THREADS, 0, p->stream>>>(st->adj_off, st->adj_idx, n, (double)st->prm.lambda, st->cg_p, st->cg_Ap,
+                                                           st->part_a, st->cg_sc);
+        dm_k_cg_update_x<<<nb, DM_SH_THREADS, 0, p->stream>>>(n, st->cg_p, st->cg_Ap, x_dev, st->cg_r, st->part_a, st->part_b, nb,
+                                                               st->cg_sc);
+        dm_k_cg_update_p<<<nb, DM_SH_THREADS, 0, p->stream>>>(n, st->cg_r, st->cg_p, st->part_b, nb, st->cg_sc, st->rr_next);
+        dm_k_cg_advance<<<1, 1, 0, p->stream>>>(st->cg_sc, st->rr_next, tol2);
+        rc = check_launch(p, 4);
+    }
+    return rc;
+}
+
+// out = (I + lambda L)^-2 g: two solves (reading R27); the result stays in st->cg_x (fp64)
+int shape_precondition(dm_plan* p, dm_shape_state* st, const float* g_dev)
+{
+    int rc = shape_cg_solve<float>(p, st, g_dev, st->cg_y);
+    if (rc) return rc;
+    return shape_cg_solve<double>(p, st, st->cg_y, st->cg_x);
+}
+
+}  // namespace
+
+extern "C" {
+
+int dm_shape_params_default(dm_shape_params* out)
+{
+    if (!out) return DM_ERR_INVALID_ARG;
+    out->lr = 1e-3f;
+    out->lambda = 50.0f;
+    out->beta1 = 0.9f;
+    out->beta2 = 0.999f;
+    out->eps = 1e-8f;
+    out->cg_tol = 1e-7f;
+    out->cg_max_iter = 400;
+    return DM_OK;
+}
+
+int dm_shape_state_create(dm_plan* p, const dm_shape_params* params, dm_shape_state** out)
+{
+    if (!out) return DM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!p) return DM_ERR_INVALID_ARG;
+    dm_shape_params prm;
+    dm_shape_params_default(&prm);
+    if (params) prm = *params;
+    if (!(prm.lr > 0.f) || !(prm.lambda >= 0.f) || !(prm.beta1 >= 0.f && prm.beta1 < 1.f) || !(prm.beta2 >= 0.f && prm.beta2 < 1.f) ||
+        !(prm.eps >= 0.f) || !(prm.cg_tol > 0.f) || prm.cg_max_iter < 1 || !std::isfinite(prm.lr) || !std::isfinite(prm.lambda))
+        return DM_ERR_INVALID_ARG;
+    dm_shape_state* st = new (std::nothrow) dm_shape_state();
+    if (!st) return DM_ERR_ALLOC;
+    st->plan = p;
+    st->prm = prm;
+    const int n = p->n_vertices;
+    st->n_blocks = (n + DM_SH_THREADS - 1) / DM_SH_THREADS;
+    int rc = DM_OK;
+    do {
+        // the vertex graph: distinct neighbours of every vertex, ascending
+        std::vector<int32_t> off, idx;
+        try {
+            std::vector<std::pair<int32_t, int32_t>> e;
+            e.reserve((size_t)p->n_faces * 6);
+            for (int32_t t = 0; t < p->n_faces; ++t)
+                for (int a = 0; a < 3; ++a) {
+                    const int32_t i = p->faces_host[3 * (size_t)t + a], j = p->faces_host[3 * (size_t)t + (a + 1) % 3];
+                    if (i != j) {
+                        e.emplace_back(i, j);
+                        e.emplace_back(j, i);
+                    }
+                }
+            std::sort(e.begin(), e.end());
+            e.erase(std::unique(e.begin(), e.end()), e.end());
+            off.assign((size_t)n + 1, 0);
+            idx.resize(e.size());
+            for (size_t q = 0; q < e.size(); ++q) {
+                off[(size_t)e[q].first + 1]++;
+                idx[q] = e[q].second;
+            }
+            for (int v = 0; v < n; ++v) off[(size_t)v + 1] += off[v];
+        } catch (...) { rc = DM_ERR_ALLOC; break; }
+        const size_t n3 = (size_t)n * 3, nvox = (size_t)p->gd.nx * p->gd.ny * p->gd.nz, nb3 = (size_t)st->n_blocks * 3;
+        if (cudaMalloc(&st->adj_off, off.size() * sizeof(int32_t)) != cudaSuccess ||
+            cudaMalloc(&st->adj_idx, std::max<size_t>(1, idx.size()) * sizeof(int32_t)) != cudaSuccess ||
+            cudaMalloc(&st->cg_x, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->cg_y, n3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->cg_r, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->cg_p, n3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->cg_Ap, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->part_a, nb3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->part_b, nb3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->rr_next, 3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->cg_sc, sizeof(DmCgScalars)) != cudaSuccess || cudaMalloc(&st->mom, n3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->amax_part, DM_SH_LOSS_BLOCKS * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->s_next, sizeof(double)) != cudaSuccess || cudaMalloc(&st->adam, sizeof(DmAdamScalars)) != cudaSuccess ||
+            cudaMalloc(&st->image, nvox * sizeof(float)) != cudaSuccess || cudaMalloc(&st->cot, nvox * sizeof(float)) != cudaSuccess ||
+            cudaMalloc(&st->grad, n3 * sizeof(float)) != cudaSuccess ||
+            cudaMalloc(&st->loss_part, DM_SH_LOSS_BLOCKS * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->loss, sizeof(double)) != cudaSuccess) { rc = DM_ERR_ALLOC; break; }
+        if (cudaMemcpyAsync(st->adj_off, off.data(), off.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) != cudaSuccess ||
+            (!idx.empty() && cudaMemcpyAsync(st->adj_idx, idx.data(), idx.size() * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream) !=
+                                 cudaSuccess) ||
+            cudaMemsetAsync(st->mom, 0, n3 * sizeof(double), p->stream) != cudaSuccess ||
+            cudaMemsetAsync(st->adam, 0, sizeof(DmAdamScalars), p->stream) != cudaSuccess ||
+            cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+    } while (0);
+    if (rc != DM_OK) {
+        dm_shape_state_destroy(st);
+        cudaGetLastError();
+        return rc;
+    }
+    *out = st;
+    return DM_OK;
+}
+
+int dm_shape_precondition(dm_plan* p, dm_shape_state* st, const float* g_dev, float* out_dev)
+{
+    if (!p || !st || st->plan != p || !g_dev || !out_dev) return DM_ERR_INVALID_ARG;
+    int rc = shape_precondition(p, st, g_dev);
+    if (rc) return rc;
+    const int n3 = p->n_vertices * 3;
+    dm_k_f64_to_f32<<<(n3 + 255) / 256, 256, 0, p->stream>>>(st->cg_x, n3, out_dev);
+    return check_launch(p);
+}
+
+int dm_shape_step(dm_plan* p, dm_shape_state* st, float* vertices_dev, const float* target_dev, const float* psf_cov_host,
+                  double* loss_host)
+{
+    if (!p || !st || st->plan != p || !vertices_dev || !target_dev || !psf_cov_host) return DM_ERR_INVALID_ARG;
+    int rc = dm_render(p, vertices_dev, psf_cov_host, st->image);
+    if (rc) return rc;
+    const long long nvox = (long long)p->gd.nx * p->gd.ny * p->gd.nz;
+    dm_k_shape_loss<<<DM_SH_LOSS_BLOCKS, DM_SH_THREADS, 0, p->stream>>>(st->image, target_dev, nvox, st->cot, st->loss_part);
+    dm_k_shape_loss_final<<<1, DM_SH_THREADS, 0, p->stream>>>(st->loss_part, DM_SH_LOSS_BLOCKS, st->loss);
+    if ((rc = check_launch(p, 2))) return rc;
+    // the vertices are the ones of the render above: its spectrum may be reused whatever DM_OPT_REUSE_SPECTRUM says
+    const bool reuse_saved = p->reuse_F;
+    p->reuse_F = true;
+    rc = dm_render_backward(p, vertices_dev, psf_cov_host, st->cot, st->grad, nullptr);
+    p->reuse_F = reuse_saved;
+    if (rc) return rc;
+    if ((rc = shape_precondition(p, st, st->grad))) return rc;
+    const int n3 = p->n_vertices * 3;
+    dm_k_adam_max<<<DM_SH_LOSS_BLOCKS, DM_SH_THREADS, 0, p->stream>>>(st->cg_x, n3, st->amax_part);
+    dm_k_adam_update<<<(n3 + DM_SH_THREADS - 1) / DM_SH_THREADS, DM_SH_THREADS, 0, p->stream>>>(
+        st->cg_x, n3, st->amax_part, DM_SH_LOSS_BLOCKS, st->mom, vertices_dev, st->adam, (double)st->prm.lr, (double)st->prm.beta1,
+        (double)st->prm.beta2, (double)st->prm.eps, st->s_next);
+    dm_k_adam_advance<<<1, 1, 0, p->stream>>>(st->adam, st->s_next);
+    if ((rc = check_launch(p, 3))) return rc;
+    p->F_valid = false;   // the vertices moved
+    if (loss_host) {
+        if (cudaMemcpyAsync(loss_host, st->loss, sizeof(double), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+            cudaStreamSynchronize(p->stream) != cudaSuccess)
+            return DM_ERR_CUDA;
+    }
+    return DM_OK;
+}
+
+void dm_shape_state_destroy(dm_shape_state* st)
+{
+    if (!st) return;
+    cudaFree(st->adj_off);
+    cudaFree(st->adj_idx);
+    cudaFree(st->cg_x);
+    cudaFree(st->cg_y);
+    cudaFree(st->cg_r);
+    cudaFree(st->cg_p);
+    cudaFree(st->cg_Ap);
+    cudaFree(st->part_a);
+    cudaFree(st->part_b);
+    cudaFree(st->rr_next);
+    cudaFree(st->cg_sc);
+    cudaFree(st->mom);
+    cudaFree(st->amax_part);
+    cudaFree(st->s_next);
+    cudaFree(st->adam);
+    cudaFree(st->image);
+    cudaFree(st->cot);
+    cudaFree(st->grad);
+    cudaFree(st->loss_part);
+    cudaFree(st->loss);
+    delete st;
 }
 
 }  // extern "C"

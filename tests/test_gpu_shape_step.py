@@ -1,0 +1,95 @@
+"""GPU parity of the shape-optimisation step (eq. 17; NEXT 4 of SURVEY.md section 8(f)) against
+oracle/shape_step.py: the (I + lambda L)^-2 preconditioner on its own (device conjugate gradients against dense solves),
+three consecutive steps on a <= 200-vertex mesh, and ten steps at config 4 whose loss must fall."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import build_workload
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dm():
+    import torch
+    import paper_2303_10440_b200 as dm
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    dm.load_library()
+    return dm
+
+
+def _rel(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+@pytest.mark.parametrize("cfg,sub", [(1, None), (2, 2), (3, 1)])
+def test_preconditioner_against_dense_solves(dm, cfg, sub):
+    """One sphere (162 vertices), a perturbed sphere and an aggregate of 8 components (8 zero modes of L)."""
+    import torch
+    w = build_workload(cfg, subdiv_override=sub, grid_override=(8, 8, 8))
+    plan = dm.Plan(w.n, w.spacing, w.origin, w.mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    g = np.random.default_rng(5).standard_normal(w.vertices.shape).astype(np.float32)
+    L = oracle.connectivity_laplacian(w.faces, len(w.vertices))
+    for lam in (50.0, 3.0, 0.0):
+        st = plan.shape_state(lambda_=lam)
+        out = st.precondition(torch.as_tensor(g, device="cuda")).cpu().numpy()
+        ref = oracle.precondition(g.astype(np.float64), L, lam)
+        err = _rel(out, ref)
+        print(f"cfg{cfg} n_V={len(w.vertices)} lambda={lam}: preconditioner rel L2 error {err:.2e}")
+        assert err <= 1e-5
+        out2 = st.precondition(torch.as_tensor(g, device="cuda")).cpu().numpy()
+        assert np.array_equal(out, out2)                     # fixed-order reductions: bitwise reproducible
+        st.close()
+    plan.close()
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_three_shape_steps_against_the_oracle(dm, mode):
+    import torch
+    w = build_workload(1, grid_override=(24, 24, 24))                 # 162 vertices, 320 triangles
+    wt = build_workload(2, subdiv_override=2, grid_override=(24, 24, 24))   # target: a perturbed sphere of radius 0.35
+    cov = (np.array([1.2, 1.2, 2.0]) * np.array(w.spacing)) ** 2
+    cov = np.array([cov[0], cov[1], cov[2], 0.0, 0.0, 0.0])
+    target = oracle.render(wt.vertices, wt.faces, w.n, w.spacing, w.origin, cov, mode)
+    plan = dm.Plan(w.n, w.spacing, w.origin, mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    lr = 2e-3
+    st = plan.shape_state(lr=lr)
+    ost = oracle.ShapeState()
+    prm = oracle.ShapeParams(lr=lr)
+    vd = torch.as_tensor(w.vertices, device="cuda").clone()
+    td = torch.as_tensor(target.astype(np.float32), device="cuda")
+    v_o = w.vertices.astype(np.float64)
+    for step in range(3):
+        v_before = vd.cpu().numpy().astype(np.float64)
+        loss = st.step(vd, td, cov, return_loss=True)
+        v_new_o, loss_o = oracle.shape_step(v_o.astype(np.float32), w.faces, w.n, w.spacing, w.origin, cov, mode,
+                                            target.astype(np.float32), ost, prm)
+        v_gpu = vd.cpu().numpy().astype(np.float64)
+        e_v = _rel(v_gpu, v_new_o)
+        e_d = _rel(v_gpu - v_before, v_new_o - v_o.astype(np.float32).astype(np.float64))
+        e_l = abs(loss - loss_o) / abs(loss_o)
+        print(f"mode {mode} step {step}: vertices rel {e_v:.2e}, displacement rel {e_d:.2e}, Phi_1 rel {e_l:.2e}")
+        assert e_v <= 1e-4
+        assert e_d <= 5e-3
+        assert e_l <= 1e-3
+        assert np.abs(v_gpu - v_before).max() <= lr * 1.0001 + 1e-7      # AdamUniform: no coordinate moves more than lr
+        v_o = v_new_o
+    plan.close()
+
+
+def test_cfg4_ten_shape_steps_decrease_phi1(dm):
+    import torch
+    w = build_workload(4)
+    wt = build_workload(4, seed_offset=100)
+    plan = dm.Plan(w.n, w.spacing, w.origin, w.mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    target = plan.render(torch.as_tensor(wt.vertices, device="cuda"), w.psf_cov).clone()
+    plan.set_narrow_band(w.psf_cov, 0.01)                      # the shape step runs on the narrow band
+    st = plan.shape_state(lr=2e-4)
+    vd = torch.as_tensor(w.vertices, device="cuda").clone()
+    losses = [st.step(vd, target, w.psf_cov, return_loss=True) for _ in range(10)]
+    print("cfg4 shape steps, Phi_1:", " ".join(f"{x:.4e}" for x in losses))
+    assert np.isfinite(losses).all() and torch.isfinite(vd).all()
+    assert losses[-1] < losses[0] and sum(b < a for a, b in zip(losses, losses[1:])) >= 8
+    st.close()
+    plan.close()
