@@ -107,6 +107,65 @@ def oracle_sample(w, n_freq: int, seed: int = 0):
     return {"pairs": pairs, "fwd_s": t1 - t0, "bwd_s": t2 - t1, "n_freq": int(len(idx)), "cores": oracle.num_threads()}
 
 
+def oracle_sample_single_thread(cfg: int, n_freq: int):
+    """The same sample with the oracle's OpenMP loop on ONE thread ("once single-threaded"):
+    a child process with OMP_NUM_THREADS=1, because the thread count is fixed when libgomp starts."""
+    code = ("import json, sys; sys.path.insert(0, %r); import bench; from workloads import build_workload; "
+            "o = bench.oracle_sample(build_workload(%d), %d); print('ORACLE1 ' + json.dumps(o))" % (ROOT, cfg, n_freq))
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600, env=env).stdout
+        for line in out.splitlines():
+            if line.startswith("ORACLE1 "):
+                return json.loads(line[8:])
+    except Exception:
+        pass
+    return None
+
+
+def ncu_summary():
+    """Numbers taken from the committed ncu capture of the dominant kernel (profiles/r02_ncu_summary.json: DRAM bytes per
+    full-grid launch, issued instructions per pair, pipe utilisation), with the command that produced them.  Static
+    evidence, labelled as such; absent file = absent keys."""
+    path = os.path.join(ROOT, "profiles", "r02_ncu_summary.json")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        return json.load(f)
+
+
+def time_config(dm, cfg: int, warmup: int, steps: int):
+    """Forward / backward times of another BASELINE.json config (device-resident inputs, L2 flushed), for the extra
+    roofline entries of the JSON line."""
+    import torch
+    from workloads import build_workload
+    from workloads.configs import spectrum_cotangent
+
+    w = build_workload(cfg)
+    plan = dm.Plan(w.n, w.spacing, w.origin, w.mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    vd = torch.as_tensor(w.vertices, device="cuda")
+    Gd = torch.as_tensor(spectrum_cotangent(w), device="cuda")
+    F = torch.empty(w.spectrum_shape, dtype=torch.complex64, device="cuda")
+    dv = torch.empty((w.vertices.shape[0], 3), dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    fw, bw, bk = [], [], []
+    for it in range(warmup + steps):
+        flush.fill_(1)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record()
+        plan.mesh_ft_forward(vd, out=F)
+        ev[1].record()
+        plan.mesh_ft_backward(vd, Gd, out=dv)
+        ev[2].record()
+        k = plan.stage_ms()["mesh_ft"]
+        if it >= warmup:
+            fw.append(ev[0].elapsed_time(ev[1]))
+            bw.append(ev[1].elapsed_time(ev[2]))
+            bk.append(k)
+    plan.close()
+    return w, float(np.median(fw)), float(np.median(bw)), float(np.median(bk))
+
+
 def run_reference(args):
     """The reference arm of this tier = the oracle, timed on host cores on a bounded sample of the workload."""
     from workloads import build_workload
@@ -135,6 +194,127 @@ def run_reference(args):
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+def run_sharded(args):
+    """--shard slab: ONE problem (config --cfg) whose stored spectrum is sharded over the ranks by x-slab (SURVEY.md
+    section 8(e)): forward = every rank's rows + one all-gather of F, backward = every rank's rows +
+    one all-reduce of dL/dv (NCCL).  Strong scaling: value = the problem's pairs / max-over-ranks time."""
+    import torch
+    import torch.distributed as dist
+
+    import paper_2303_10440_b200 as dm
+    from paper_2303_10440_b200.sharding import sharded_mesh_ft_backward, sharded_mesh_ft_forward
+    from workloads import build_workload
+    from workloads.configs import spectrum_cotangent
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dm.load_library()
+    if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")   # which algorithm / transport (NVLS, P2P) the collectives took
+        os.environ.setdefault("NCCL_DEBUG_FILE", os.path.join(ROOT, "gpurun_out", "nccl_rank%h_%p.log"))
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    w = build_workload(args.cfg)                      # the same mesh on every rank
+    plan = dm.Plan(w.n, w.spacing, w.origin, w.mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    vd = torch.as_tensor(w.vertices, device="cuda")
+    Gd = torch.as_tensor(spectrum_cotangent(w), device="cuda")
+    F = torch.zeros(w.spectrum_shape, dtype=torch.complex64, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    hv = torch.as_tensor(w.vertices).pin_memory()
+    hg = torch.as_tensor(np.random.default_rng(10 + w.seed).standard_normal(w.n).astype(np.float32)).pin_memory()
+    himg = torch.empty(w.n, dtype=torch.float32).pin_memory()
+    hdv = torch.empty((w.vertices.shape[0], 3), dtype=torch.float32).pin_memory()
+    gimg = torch.empty(w.n, dtype=torch.float32, device="cuda")
+    ggrad = torch.empty(w.n, dtype=torch.float32, device="cuda")
+    Gimg = torch.empty(w.spectrum_shape, dtype=torch.complex64, device="cuda")
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step(ev):
+        flush.fill_(1)
+        ev[0].record(stream)
+        sharded_mesh_ft_forward(plan, vd, out=F)
+        ev[1].record(stream)
+        dv = sharded_mesh_ft_backward(plan, vd, Gd)
+        ev[2].record(stream)
+        return dv
+
+    def e2e_step():
+        vd.copy_(hv, non_blocking=True)
+        ggrad.copy_(hg, non_blocking=True)
+        sharded_mesh_ft_forward(plan, vd, out=F)
+        plan.spectrum_to_image(F, w.psf_cov, out=gimg)
+        himg.copy_(gimg, non_blocking=True)
+        plan.image_to_spectrum_cotangent(ggrad, w.psf_cov, out=Gimg)
+        hdv.copy_(sharded_mesh_ft_backward(plan, vd, Gimg), non_blocking=True)
+
+    def new_ev():
+        return [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+
+    for _ in range(max(args.warmup, 0)):
+        step(new_ev())
+    launches0 = plan.launch_count()
+    barrier()
+    evs = [new_ev() for _ in range(args.steps)]
+    with ClockSampler(local) as clk:
+        for ev in evs:
+            step(ev)
+        barrier()
+    launches = plan.launch_count() - launches0
+    fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    bwd_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    e2e_step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2e_n = max(1, min(args.steps, 3))
+    e0.record(stream)
+    for _ in range(e2e_n):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    t = torch.tensor([fwd_ms + bwd_ms, fwd_ms, bwd_ms, e0.elapsed_time(e1) / e2e_n], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    step_ms, fwd_ms, bwd_ms, e2e_ms = (float(x) for x in t.tolist())
+    if rank == 0:
+        sm_max_mhz, peak_src = _peaks()
+        n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+        peak = FP32_LANES_PER_CLK_PER_SM * n_sm * sm_max_mhz * 1e6 / 1e12 * world
+        pairs = float(w.pairs)
+        achieved = FLOOR_OPS["bwd"][w.mode] * pairs / (bwd_ms * 1e-3) / 1e12
+        line = {
+            "metric": METRIC, "value": pairs / (step_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "cfg": w.cfg, "mode": "surface" if w.mode else "volume",
+                       "n_triangles": int(w.faces.shape[0]), "grid": list(w.n), "pairs_per_pass": pairs,
+                       "l2": "flushed between timed iterations (256 MB write)",
+                       "parallelism": f"x-slab of the stored spectrum over {world} rank(s); all-gather of F, all-reduce of dL/dv"},
+            "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
+            "e2e": {"value": pairs / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                    "h2d_bytes_per_step": hv.numel() * 4 + hg.numel() * 4, "d2h_bytes_per_step": himg.numel() * 4 + hdv.numel() * 4,
+                    "what": "sharded forward + all-gather + image stage, cotangent stage + sharded backward + all-reduce, "
+                            "pinned host buffers in and out on every rank"},
+            "gpu_launches": int(launches), "clocks": clk.summary(),
+            "roofline": {"bound": "alu", "kernel": "dm_k_backward_fast + all-reduce (whole sharded backward)",
+                         "achieved": achieved, "peak": peak, "unit": "T lane-op/s over all ranks", "frac": achieved / peak,
+                         "traffic": None, "peak_source": f"{world} x 128 x {n_sm} SMs x {sm_max_mhz:.0f} MHz ({peak_src})"},
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
 
 
 def run_ours(args):
@@ -277,22 +457,41 @@ def run_ours(args):
         bk_ms = float(np.mean(bwd_kernel_ms))
         achieved = FLOOR_OPS["bwd"][w.mode] * pairs / (bk_ms * 1e-3) / 1e12
         sm_mhz = clocks.get("sm_mhz") or sm_max_mhz
+        ncu = ncu_summary()
         roofline = {
-            "bound": "alu", "kernel": "dm_k_backward (A6, dominant)", "achieved": achieved, "peak": peak,
-            "unit": "T lane-op/s (FP32 issue: 128 lanes/clk/SM)", "frac": achieved / peak, "traffic": None,
-            "traffic_note": "ncu --set full needs an x-slab launch for valid counters: 12.2 MB DRAM per 1.36e10-pair launch "
-                            "(profiles/r01f_ncu_fast_kernels.txt); the kernel is compute-bound",
+            "bound": "alu", "kernel": "dm_k_backward_fast (A6, dominant)", "achieved": achieved, "peak": peak,
+            "unit": "T lane-op/s (FP32 issue: 128 lanes/clk/SM)", "frac": achieved / peak,
+            "traffic": (ncu or {}).get("dram_bytes_per_full_grid_launch"),
             "peak_source": f"128 x {n_sm} SMs x {sm_max_mhz:.0f} MHz ({peak_src}); DESIGN.md section 7",
             "frac_at_measured_clock": achieved / (peak * sm_mhz / sm_max_mhz),
             "algorithmic_ops_per_pair": FLOOR_OPS["bwd"][w.mode], "kernel_ms": bk_ms,
-            "ncu": {"issued_instr_per_pair": 85.8, "issue_active_pct": 79.5, "source": "profiles/r01f_ncu_fast_kernels.txt "
-                    "(cfg 4 x-slab capture; static numbers, not measured by this run)"},
             "forward": {"achieved": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12,
                         "frac": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12 / peak,
                         "algorithmic_ops_per_pair": FLOOR_OPS["fwd"][w.mode]},
         }
+        if ncu:
+            roofline["ncu"] = ncu
+        # the other full-size configs (volume mode carries 5 more operations per pair against the same floor)
+        extra = {}
+        for c in [int(x) for x in args.extra_cfgs.split(",") if x.strip()]:
+            if c == w.cfg or world > 1:
+                continue
+            wc, f_ms, b_ms, k_ms = time_config(dm, c, 1, 2 if c < 5 else 1)
+            pc = float(wc.pairs)
+            extra[f"cfg{c}"] = {
+                "mode": "surface" if wc.mode else "volume", "pairs_per_pass": pc, "fwd_ms": f_ms, "bwd_ms": b_ms,
+                "bwd_kernel_ms": k_ms, "fwd_bwd_pairs_s": pc / ((f_ms + b_ms) * 1e-3),
+                "frac_backward": FLOOR_OPS["bwd"][wc.mode] * pc / (k_ms * 1e-3) / 1e12 / peak,
+                "frac_forward": FLOOR_OPS["fwd"][wc.mode] * pc / (f_ms * 1e-3) / 1e12 / peak}
+        roofline["other_configs"] = extra
         o = oracle_sample(w, args.ref_freqs)
+        o1 = oracle_sample_single_thread(w.cfg, max(8, args.ref_freqs // 8))
         sample = f"{o['n_freq']} random stored frequencies x all {w.faces.shape[0]} triangles, forward+backward"
+        # the CPU image stage (PSF multiply + numpy irfftn, fp64) on this grid, for the "ms per render" stage split
+        import oracle as _oracle
+        t0 = time.perf_counter()
+        _oracle.spectrum_to_image(F.cpu().numpy(), w.n, w.spacing, w.origin, w.psf_cov.astype(np.float64))
+        cpu_image_stage_ms = (time.perf_counter() - t0) * 1e3
         line = {
             "metric": METRIC, "value": world * pairs / (step_ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True,
@@ -310,7 +509,13 @@ def run_ours(args):
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
             "cpu_baseline": {"value": o["pairs"] / (o["fwd_s"] + o["bwd_s"]), "unit": UNIT, "cores": o["cores"],
                              "kind": "oracle", "sample": sample, "fwd_pairs_s": o["pairs"] / o["fwd_s"],
-                             "bwd_pairs_s": o["pairs"] / o["bwd_s"]},
+                             "bwd_pairs_s": o["pairs"] / o["bwd_s"],
+                             "single_thread": None if o1 is None else {
+                                 "value": o1["pairs"] / (o1["fwd_s"] + o1["bwd_s"]), "cores": o1["cores"],
+                                 "sample": f"{o1['n_freq']} random stored frequencies x all triangles",
+                                 "fwd_pairs_s": o1["pairs"] / o1["fwd_s"], "bwd_pairs_s": o1["pairs"] / o1["bwd_s"]},
+                             "image_stage_ms": cpu_image_stage_ms,
+                             "image_stage": "PSF multiply + numpy irfftn (fp64) of one spectrum of this grid"},
             "narrow_band": nb, "wall_s_timed_region": t_wall,
         }
         print(json.dumps(line), flush=True)
@@ -327,11 +532,18 @@ def main():
     ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json config 1..5 (default 4, the target config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-freqs", type=int, default=192, help="stored frequencies per oracle sample")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"],
+                    help="replicas (default): every rank its own problem, weak scaling, no data-path collective; slab: ONE problem "
+                         "sharded by x-slab of the stored spectrum (all-gather of F, all-reduce of dL/dv), strong scaling")
+    ap.add_argument("--extra-cfgs", default="3,5", help="other BASELINE.json configs timed (N=1 only) for the extra roofline "
+                    "entries; '' switches them off")
     ap.add_argument("--x-slab", default="", help="a:b -- profiling aid (ncu counters overflow on the 0.4 s full-grid launch): run "
                     "forward/backward on rows [a,b) of the spectrum only and print a short line that is NOT a bench result")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.shard == "slab":
+        run_sharded(args)
     else:
         run_ours(args)
 

@@ -44,3 +44,48 @@ def sharded_mesh_ft_backward(plan, vertices, dL_dF, group=None):
 
         dv = torch.zeros((plan.n_vertices, 3), dtype=torch.float32, device=plan.device)
     return allreduce_vertex_gradient(dv, group)
+
+
+def allgather_spectrum_slabs(F, group=None):
+    """All-gather of the x-slabs of a spectrum tensor F [n_x, n_y, n_z/2+1] (complex or real, CPU or CUDA), in place:
+    on entry every rank holds valid rows ``slab_bounds(n_x, world, rank)`` of F, on return every rank holds all rows.
+    Needed only when a rank goes on to the inverse FFT.  Slabs differ by at most one row, so they
+    are padded to the largest and exchanged with ONE all_gather_into_tensor (<= 68 MB at config 5)."""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
+        return F
+    world, rank = dist.get_world_size(group), dist.get_rank(group)
+    n_x = F.shape[0]
+    rows = max(slab_bounds(n_x, world, r)[1] - slab_bounds(n_x, world, r)[0] for r in range(world))
+    Fr = torch.view_as_real(F) if F.is_complex() else F
+    send = torch.zeros((rows,) + tuple(Fr.shape[1:]), dtype=Fr.dtype, device=Fr.device)
+    b, e = slab_bounds(n_x, world, rank)
+    send[: e - b] = Fr[b:e]
+    recv = torch.empty((world * rows,) + tuple(Fr.shape[1:]), dtype=Fr.dtype, device=Fr.device)
+    dist.all_gather_into_tensor(recv, send, group=group)
+    for r in range(world):
+        rb, re_ = slab_bounds(n_x, world, r)
+        if r != rank and re_ > rb:
+            Fr[rb:re_] = recv[r * rows: r * rows + (re_ - rb)]
+    return F
+
+
+def sharded_mesh_ft_forward(plan, vertices, out=None, group=None, gather=True):
+    """F with the stored spectrum sharded over the ranks of ``group`` by x-slab: every rank evaluates its own rows in the
+    CUDA kernels (no communication: the frequencies are independent); with ``gather`` the slabs are then all-gathered so
+    that every rank holds the whole spectrum."""
+    import torch
+    import torch.distributed as dist
+
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    begin, end = slab_bounds(plan.n[0], world, rank)
+    if out is None:
+        out = torch.zeros(plan.spectrum_shape, dtype=torch.complex64, device=plan.device)
+    if end > begin:
+        plan.set_slab(begin, end)
+        plan.mesh_ft_forward(vertices, out=out)
+        plan.set_slab(0, plan.n[0])
+    return allgather_spectrum_slabs(out, group) if gather else out

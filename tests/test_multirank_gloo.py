@@ -13,7 +13,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2303_10440_b200.sharding import allreduce_vertex_gradient, slab_bounds
+from paper_2303_10440_b200.sharding import allgather_spectrum_slabs, allreduce_vertex_gradient, slab_bounds
 
 
 def test_slab_bounds_tile_the_grid():
@@ -67,6 +67,11 @@ def _worker(rank, world, port, out_dir):
             Fs[idx] = torch.as_tensor(Fslab)
             Fr = torch.view_as_real(Fs).clone()
             dist.all_reduce(Fr)
+            # ... and through the library's own helper (padded slabs, one all_gather_into_tensor)
+            Fg = torch.full((nx, ny, nzh), float("nan"), dtype=torch.complex128)
+            Fg[b:e] = torch.as_tensor(Fslab).reshape(e - b, ny, nzh)
+            allgather_spectrum_slabs(Fg)
+            np.save(os.path.join(out_dir, f"Fg_{mode}_{rank}.npy"), Fg.numpy())
             np.save(os.path.join(out_dir, f"dv_{mode}_{rank}.npy"), dv.numpy())
             np.save(os.path.join(out_dir, f"F_{mode}_{rank}.npy"), torch.view_as_complex(Fr).numpy())
     finally:
@@ -90,3 +95,5 @@ def test_sharded_backward_allreduce_matches_whole_grid(world, tmp_path):
             assert np.linalg.norm(dv - ref) <= 1e-12 * np.linalg.norm(ref)
             F = np.load(tmp_path / f"F_{mode}_{r}.npy")
             assert np.abs(F - Fref).max() <= 1e-12 * abs(Fref[0])
+            Fg = np.load(tmp_path / f"Fg_{mode}_{r}.npy").reshape(-1)
+            assert np.isfinite(Fg).all() and np.abs(Fg - Fref).max() <= 1e-12 * abs(Fref[0])
