@@ -204,7 +204,8 @@ typedef struct dm_shape_params {
     float   beta2;       /* second-moment decay (default 0.999)                                       */
     float   eps;         /* default 1e-8                                                              */
     float   cg_tol;      /* a solve stops when |r| <= cg_tol |b| on every column (default 1e-7)       */
-    int32_t cg_max_iter; /* launches are queued for this many iterations per solve (default 400)      */
+    int32_t cg_max_iter; /* at most this many iterations are queued per solve (default 400); fewer when
+                            the convergence bound of CG for cond(I + lambda L) <= 1 + 2 lambda d_max says so */
 } dm_shape_params;
 
 int dm_shape_params_default(dm_shape_params* out);

@@ -964,8 +964,9 @@ struct dm_shape_state {
     int n_blocks = 0;                // ceil(n_vertices / DM_SH_THREADS)
     int32_t *adj_off = nullptr, *adj_idx = nullptr;   // CSR of the distinct neighbours of every vertex (L = D - A)
     double *cg_x = nullptr, *cg_y = nullptr, *cg_r = nullptr, *cg_p = nullptr, *cg_Ap = nullptr;
-    double *part_a = nullptr, *part_b = nullptr, *rr_next = nullptr;
-    DmCgScalars* cg_sc = nullptr;
+    double *part_a = nullptr, *part_b = nullptr;
+    DmCgScalars* cg_sc = nullptr;    // [2]: the scalars of the current and of the next iteration
+    int cg_iter_bound = 0;           // iterations after which CG has converged to cg_tol whatever the right-hand side
     double *mom = nullptr, *amax_part = nullptr, *s_next = nullptr;
     DmAdamScalars* adam = nullptr;
     float *image = nullptr, *cot = nullptr, *grad = nullptr;
@@ -983,14 +984,15 @@ int shape_cg_solve(dm_plan* p, dm_shape_state* st, const TB* b_dev, double* x_de
     dm_k_cg_init_final<<<1, DM_SH_THREADS, 0, p->stream>>>(st->part_a, nb, st->cg_sc);
     int rc = check_launch(p, 2);
     const double tol2 = (double)st->prm.cg_tol * (double)st->prm.cg_tol;
-    for (int it = 0; it < st->prm.cg_max_iter && rc == DM_OK; ++it) {
+    const int n_iter = std::min(st->prm.cg_max_iter, st->cg_iter_bound);
+    for (int it = 0; it < n_iter && rc == DM_OK; ++it) {
+        const DmCgScalars* sc = st->cg_sc + (it & 1);
+        DmCgScalars* sc_next = st->cg_sc + ((it + 1) & 1);
         dm_k_cg_spmv<<<nb, DM_SH_THREADS, 0, p->stream>>>(st->adj_off, st->adj_idx, n, (double)st->prm.lambda, st->cg_p, st->cg_Ap,
-                                                           st->part_a, st->cg_sc);
-        dm_k_cg_update_x<<<nb, DM_SH_THREADS, 0, p->stream>>>(n, st->cg_p, st->cg_Ap, x_dev, st->cg_r, st->part_a, st->part_b, nb,
-                                                               st->cg_sc);
-        dm_k_cg_update_p<<<nb, DM_SH_THREADS, 0, p->stream>>>(n, st->cg_r, st->cg_p, st->part_b, nb, st->cg_sc, st->rr_next);
-        dm_k_cg_advance<<<1, 1, 0, p->stream>>>(st->cg_sc, st->rr_next, tol2);
-        rc = check_launch(p, 4);
+                                                           st->part_a, sc);
+        dm_k_cg_update_x<<<nb, DM_SH_THREADS, 0, p->stream>>>(n, st->cg_p, st->cg_Ap, x_dev, st->cg_r, st->part_a, st->part_b, nb, sc);
+        dm_k_cg_update_p<<<nb, DM_SH_THREADS, 0, p->stream>>>(n, st->cg_r, st->cg_p, st->part_b, nb, sc, sc_next, tol2);
+        rc = check_launch(p, 3);
     }
     return rc;
 }
@@ -1060,7 +1062,17 @@ int dm_shape_state_create(dm_plan* p, const dm_shape_params* params, dm_shape_st
                 off[(size_t)e[q].first + 1]++;
                 idx[q] = e[q].second;
             }
-            for (int v = 0; v < n; ++v) off[(size_t)v + 1] += off[v];
+            int dmax = 0;
+            for (int v = 0; v < n; ++v) {
+                dmax = std::max(dmax, (int)off[(size_t)v + 1]);
+                off[(size_t)v + 1] += off[v];
+            }
+            // CG on a symmetric positive definite matrix of condition number kappa reduces the A-norm of the error by
+            // 2 ((sqrt(kappa)-1)/(sqrt(kappa)+1))^k; here 1 <= eig(I + lambda L) <= 1 + 2 lambda d_max (Gershgorin), so
+            // k = 1/2 sqrt(kappa) ln(2 sqrt(kappa) / tol) iterations reach cg_tol in the 2-norm too: queue no more than
+            // that (+ 10 %), the launches after convergence being no-ops that still cost their launch
+            const double kap = 1.0 + 2.0 * (double)prm.lambda * (double)dmax;
+            st->cg_iter_bound = (int)std::ceil(1.1 * 0.5 * std::sqrt(kap) * std::log(2.0 * std::sqrt(kap) / (double)prm.cg_tol)) + 2;
         } catch (...) { rc = DM_ERR_ALLOC; break; }
         const size_t n3 = (size_t)n * 3, nvox = (size_t)p->gd.nx * p->gd.ny * p->gd.nz, nb3 = (size_t)st->n_blocks * 3;
         if (cudaMalloc(&st->adj_off, off.size() * sizeof(int32_t)) != cudaSuccess ||
@@ -1068,8 +1080,8 @@ int dm_shape_state_create(dm_plan* p, const dm_shape_params* params, dm_shape_st
             cudaMalloc(&st->cg_x, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->cg_y, n3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->cg_r, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->cg_p, n3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->cg_Ap, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->part_a, nb3 * sizeof(double)) != cudaSuccess ||
-            cudaMalloc(&st->part_b, nb3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->rr_next, 3 * sizeof(double)) != cudaSuccess ||
-            cudaMalloc(&st->cg_sc, sizeof(DmCgScalars)) != cudaSuccess || cudaMalloc(&st->mom, n3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->part_b, nb3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->cg_sc, 2 * sizeof(DmCgScalars)) != cudaSuccess || cudaMalloc(&st->mom, n3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->amax_part, DM_SH_LOSS_BLOCKS * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->s_next, sizeof(double)) != cudaSuccess || cudaMalloc(&st->adam, sizeof(DmAdamScalars)) != cudaSuccess ||
             cudaMalloc(&st->image, nvox * sizeof(float)) != cudaSuccess || cudaMalloc(&st->cot, nvox * sizeof(float)) != cudaSuccess ||
@@ -1147,7 +1159,6 @@ void dm_shape_state_destroy(dm_shape_state* st)
     cudaFree(st->cg_Ap);
     cudaFree(st->part_a);
     cudaFree(st->part_b);
-    cudaFree(st->rr_next);
     cudaFree(st->cg_sc);
     cudaFree(st->mom);
     cudaFree(st->amax_part);

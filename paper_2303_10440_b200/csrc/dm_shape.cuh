@@ -9,7 +9,7 @@
 // symmetric positive definite with condition number <= 1 + 2 lambda max_degree (about 700 for lambda = 50), the three
 // coordinate columns are solved at once with their own step lengths, vectors and dot products are fp64 (the work is
 // O(n_V) per iteration, nothing next to the mesh FT), and every reduction is a fixed-order two-stage tree, so the step is
-// bitwise reproducible.  One iteration = four small launches (the two dot products are grid-wide); a device flag turns the
+// bitwise reproducible.  One iteration = three small launches (the two dot products are grid-wide); a device flag turns the
 // remaining launches of a converged solve into no-ops, so the host never synchronises.
 // AdamUniform (reading R28): Adam whose second moment is one scalar per step, the largest squared gradient entry.
 #pragma once
@@ -173,13 +173,17 @@ dm_k_cg_update_x(int n, const double* __restrict__ p, const double* __restrict__
         if (threadIdx.x == 0) part_rr[3 * (size_t)blockIdx.x + c] = s;
     }
 }
-// beta = r.r(new) / r.r(old) ; p = r + beta p ; (after every block has read the old r.r) the scalars move on
+// beta = r.r(new) / r.r(old) ; p = r + beta p ; block 0 writes the scalars of the NEXT iteration into the other buffer
+// (sc_next != sc: every block may still be reading sc): the new r.r and the convergence test r.r <= tol^2 b.b on every column
 __global__ void __launch_bounds__(DM_SH_THREADS)
 dm_k_cg_update_p(int n, const double* __restrict__ r, double* __restrict__ p, const double* __restrict__ part_rr,
-                 int n_part, const DmCgScalars* __restrict__ sc, double* __restrict__ rr_next)
+                 int n_part, const DmCgScalars* __restrict__ sc, DmCgScalars* __restrict__ sc_next, double tol2)
 {
     __shared__ double sh[DM_SH_THREADS];
-    if (sc->done) return;
+    if (sc->done) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) *sc_next = *sc;
+        return;
+    }
     double rn[3];
     dm_sh_total3(part_rr, n_part, sh, rn);
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -189,19 +193,15 @@ dm_k_cg_update_p(int n, const double* __restrict__ r, double* __restrict__ p, co
             const size_t q = 3 * (size_t)i + c;
             p[q] = r[q] + beta * p[q];
         }
-    if (blockIdx.x == 0 && threadIdx.x == 0)
-        for (int c = 0; c < 3; ++c) rr_next[c] = rn[c];
-}
-// one thread: r.r <- the new value, convergence test  r.r <= tol^2 b.b  on every column
-__global__ void dm_k_cg_advance(DmCgScalars* __restrict__ sc, const double* __restrict__ rr_next, double tol2)
-{
-    if (sc->done) return;
-    bool all = true;
-    for (int c = 0; c < 3; ++c) {
-        sc->rr[c] = rr_next[c];
-        all = all && (rr_next[c] <= tol2 * sc->bb[c]);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        bool all = true;
+        for (int c = 0; c < 3; ++c) {
+            sc_next->rr[c] = rn[c];
+            sc_next->bb[c] = sc->bb[c];
+            all = all && (rn[c] <= tol2 * sc->bb[c]);
+        }
+        sc_next->done = all ? 1 : 0;
     }
-    sc->done = all ? 1 : 0;
 }
 
 // ---- AdamUniform (reading R28) -------------------------------------------------------------------------------------------
