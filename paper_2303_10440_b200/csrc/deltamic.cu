@@ -217,11 +217,11 @@ int run_forward_fast(dm_plan* p, const float* vertices_dev, float* F_dev)
         dm_k_forward_fast<0><<<grid, DM_FAST_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->gd, p->ix_begin, p->ix_end,
                                                                       n_yruns, p->tau, p->hmax2, stride, p->fwd_part);
     if ((rc = check_launch(p))) return rc;
-    // candidates of the low-k kernel: the part of its box that exists on this grid; a CTA strides over them and only
-    // the low ones (|k| h_max < DM_LOWK_RADIUS, decided on the device) cost anything
+    // candidates of the low-k kernel: the part of its box that exists on this grid, one per thread; only the low ones
+    // (|k| h_max < DM_LOWK_RADIUS, decided on the device) cost anything
     const int bx = std::min(DM_LOWK_BOX, p->gd.nx / 2), by = std::min(DM_LOWK_BOX, p->gd.ny / 2), bz = std::min(DM_LOWK_BOX, p->gd.nz / 2);
     const long long n_cand = (long long)(2 * bx + 1) * (2 * by + 1) * (bz + 1);
-    const unsigned lowk_blocks = (unsigned)std::min<long long>(n_cand, (long long)p->n_sm * 8);
+    const unsigned lowk_blocks = (unsigned)((n_cand + DM_LOWK_CAND - 1) / DM_LOWK_CAND);
     if (p->mode == DM_SURFACE)
         dm_k_forward_lowk<1><<<lowk_blocks, DM_LOWK_THREADS, 0, p->stream>>>(p->st_rec, p->st_chunk_off, p->st_n_chunks, p->gd, p->ix_begin,
                                                                  p->ix_end, bx, by, bz, p->hmax2, (float2*)F_dev);

@@ -325,11 +325,14 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
     }
 }
 
-// ---- A4 at low |k|: every pair through the robust branches; one CTA per frequency, threads stride over the records ----
-// The CTAs stride over the (2 bx + 1)(2 by + 1)(bz + 1) candidate frequencies |n_x| <= bx, |n_y| <= by, n_z <= bz (the low-k
-// box clipped to the grid); a candidate that is not "low" costs one test.  Writes F directly.  The block sum is taken in
-// a fixed order (lane tree, then the warps in order): deterministic.
+// ---- A4 at low |k|: every pair through the robust branches; one CTA per low frequency, threads stride over the records ----
+// Candidates are the (2 bx + 1)(2 by + 1)(bz + 1) frequencies |n_x| <= bx, |n_y| <= by, n_z <= bz (the low-k box clipped to the
+// grid).  Every THREAD of the grid tests one candidate (interleaved over the CTAs, so that the low ball around k = 0 is spread
+// over all of them); a CTA then evaluates the low ones it found, one after the other, with all its threads.  Each frequency
+// is written by exactly one CTA and its block sum is taken in a fixed order (lane tree, then the warps in order), so the
+// result does not depend on the order in which a CTA lists its frequencies.  grid = ceil(candidates / DM_LOWK_CAND).
 #define DM_LOWK_THREADS 256
+#define DM_LOWK_CAND 64            // candidates tested per CTA (by its first threads): enough CTAs to balance the low ones
 template <int MODE>
 __global__ void __launch_bounds__(DM_LOWK_THREADS)
 dm_k_forward_lowk(const float4* __restrict__ rec, const int32_t* __restrict__ chunk_off, int n_chunks, DmGridDev grid,
@@ -337,15 +340,29 @@ dm_k_forward_lowk(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                   float2* __restrict__ F)
 {
     __shared__ float wsum[2][DM_LOWK_THREADS / 32];
+    __shared__ int list[DM_LOWK_CAND];
+    __shared__ int n_list;
     const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
     const int Wy = 2 * by + 1, n_cand = (2 * bx + 1) * Wy * (bz + 1);
     const float hmax2 = __uint_as_float(*hmax2_bits);
-    for (int fi = blockIdx.x; fi < n_cand; fi += gridDim.x) {
+    if (threadIdx.x == 0) n_list = 0;
+    __syncthreads();
+    {
+        const int fi = (int)threadIdx.x * (int)gridDim.x + (int)blockIdx.x;
+        if (threadIdx.x < DM_LOWK_CAND && fi < n_cand) {
+            const int nz = fi % (bz + 1), nys = (fi / (bz + 1)) % Wy - by, nx = fi / ((bz + 1) * Wy) - bx;
+            const int ix = nx < 0 ? nx + grid.nx : nx;
+            const bool on_grid = !(nz > grid.nz / 2 || nys < -(grid.ny / 2) || nys > (grid.ny - 1) / 2 || nx < -(grid.nx / 2) ||
+                                   nx > (grid.nx - 1) / 2) && ix >= ix_begin && ix < ix_end;
+            if (on_grid && dm_k_is_low(grid, nx, nys, nz, hmax2) && dm_in_band(grid, nx, nys, nz)) list[atomicAdd(&n_list, 1)] = fi;
+        }
+    }
+    __syncthreads();
+    const int n_mine = n_list;
+    for (int li = 0; li < n_mine; ++li) {
+        const int fi = list[li];
         const int nz = fi % (bz + 1), nys = (fi / (bz + 1)) % Wy - by, nx = fi / ((bz + 1) * Wy) - bx;
-        if (nz > grid.nz / 2 || nys < -(grid.ny / 2) || nys > (grid.ny - 1) / 2 || nx < -(grid.nx / 2) || nx > (grid.nx - 1) / 2) continue;
         const int ix = nx < 0 ? nx + grid.nx : nx, iy = nys < 0 ? nys + grid.ny : nys;
-        if (ix < ix_begin || ix >= ix_end) continue;
-        if (!dm_k_is_low(grid, nx, nys, nz, hmax2) || !dm_in_band(grid, nx, nys, nz)) continue;
         const float kx = grid.kstep[0] * nx, ky = grid.kstep[1] * nys, kz = grid.kstep[2] * nz;
         float are = 0.f, aim = 0.f;
         for (int c = 0; c < n_chunks; ++c) {
@@ -371,7 +388,7 @@ dm_k_forward_lowk(const float4* __restrict__ rec, const int32_t* __restrict__ ch
             are += __shfl_xor_sync(0xffffffffu, are, o);
             aim += __shfl_xor_sync(0xffffffffu, aim, o);
         }
-        __syncthreads();   // the previous candidate's sums have been read
+        __syncthreads();   // the previous frequency's sums have been read
         if (lane == 0) {
             wsum[0][wrp] = are;
             wsum[1][wrp] = aim;
