@@ -558,3 +558,25 @@ def test_reuse_of_the_render_spectrum(dm):
     n2 = plan.launch_count() - n0
     assert n2 < n1 and _rel_l2(d2.cpu().numpy(), d1.cpu().numpy()) <= 1e-6
     plan.close()
+
+
+@pytest.mark.parametrize("n", [(2, 2, 4096), (4096, 1, 2), (1, 4096, 4)])
+def test_maximum_grid_extents(dm, n):
+    """The largest extent the plan accepts (4096 voxels) on each axis in turn, tiny on the others: N_z/2+1 = 2049 stored
+    z-frequencies (the 12-bit frequency field of the backward's queue entries, eight super-segments per row), 4096 rows
+    along x or y (row bookkeeping of the k-splits, fftfreq wrap of the row phases).  Surface mode, full grid vs the oracle."""
+    w = build_workload(1, grid_override=n)
+    G = spectrum_cotangent(w)
+    plan = _plan(dm, w, 1)
+    vd = _dev(w.vertices)
+    F = plan.mesh_ft_forward(vd).cpu().numpy()
+    ref = oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, 1)
+    assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0, 0, 0])
+    dv = plan.mesh_ft_backward(vd, _dev(G)).cpu().numpy()
+    assert plan.paths_used() == (0, 0)
+    dref = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, 1, G.astype(np.complex128))
+    assert _rel_l2(dv, dref) <= GRAD_TOL
+    plan.close()
+    import torch
+    with pytest.raises(dm.DeltamicError):                                # one voxel more is refused, not mis-computed
+        dm.Plan((4098, 2, 2), (1 / 4098, 0.5, 0.5), (0, 0, 0), 1, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
