@@ -188,7 +188,9 @@ void dm_plan_destroy(dm_plan* plan);
  *   g     = dPhi_1/dvertices                            through dm_render_backward
  *   g~    = (I + lambda L)^-2 g                         L = D - A, the connectivity Laplacian of the mesh's vertex graph;
  *                                                       two conjugate-gradient solves with I + lambda L on the device
- *                                                       (the paper uses a sparse Cholesky factorisation), fp64
+ *                                                       (the paper uses a sparse Cholesky factorisation), fp64; one
+ *                                                       persistent cooperative kernel per solve when the mesh fits one
+ *                                                       resident grid (~3e5 vertices), else three launches per iteration
  *   vertices <- AdamUniform(vertices, g~)               m_t = b1 m + (1-b1) g~,  s_t = b2 s + (1-b2) max_i g~_i^2,
  *                                                       v -= lr (m_t/(1-b1^t)) / (sqrt(s_t/(1-b2^t)) + eps)
  * The state owns the vertex graph, the optimiser moments (zero at creation) and all scratch; it belongs to ONE plan
@@ -206,6 +208,9 @@ typedef struct dm_shape_params {
     float   cg_tol;      /* a solve stops when |r| <= cg_tol |b| on every column (default 1e-7)       */
     int32_t cg_max_iter; /* at most this many iterations are queued per solve (default 400); fewer when
                             the convergence bound of CG for cond(I + lambda L) <= 1 + 2 lambda d_max says so */
+    int32_t solver;      /* 0 = automatic (default): one persistent cooperative kernel per solve when the whole solve
+                            fits one resident grid, else 1;  1 = three launches per iteration (same arithmetic, same
+                            results bit for bit while every vertex tile has its own block) */
 } dm_shape_params;
 
 int dm_shape_params_default(dm_shape_params* out);
@@ -215,6 +220,11 @@ int dm_shape_state_create(dm_plan* plan, const dm_shape_params* params, dm_shape
 
 /* out = (I + lambda L)^-2 g for a float32 [n_vertices*3] field g (both DEVICE pointers; they may be the same). */
 int dm_shape_precondition(dm_plan* plan, dm_shape_state* state, const float* g_dev, float* out_dev);
+
+/* Conjugate-gradient iterations the two solves of the last dm_shape_precondition / dm_shape_step took (iters[0], iters[1]);
+ * -1 when the solves ran as separate launches (meshes too large for one resident grid), which keep no count.
+ * Synchronises the stream. */
+int dm_shape_last_cg_iterations(dm_plan* plan, dm_shape_state* state, int32_t iters[2]);
 
 /* One step.  vertices_dev float32 [n_vertices*3] is updated IN PLACE; target_dev float32 [n_x*n_y*n_z] is the image m;
  * psf_cov_host as in dm_render.  loss_host = NULL, or a HOST double that receives Phi_1 of the vertices BEFORE the

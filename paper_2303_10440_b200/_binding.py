@@ -16,7 +16,7 @@ _SYMBOLS = (
     "dm_plan_create", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_mesh_ft_backward_with_spectrum", "dm_render",
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
     "dm_plan_launch_count", "dm_plan_paths_used", "dm_plan_destroy", "dm_error_string", "dm_version",
-    "dm_shape_params_default", "dm_shape_state_create", "dm_shape_precondition", "dm_shape_step", "dm_shape_state_destroy",
+    "dm_shape_params_default", "dm_shape_state_create", "dm_shape_precondition", "dm_shape_last_cg_iterations", "dm_shape_step", "dm_shape_state_destroy",
 )
 
 
@@ -29,7 +29,7 @@ class DeltamicError(RuntimeError):
 class ShapeParams(ctypes.Structure):
     """dm_shape_params (include/deltamic.h)."""
     _fields_ = [("lr", ctypes.c_float), ("lambda_", ctypes.c_float), ("beta1", ctypes.c_float), ("beta2", ctypes.c_float),
-                ("eps", ctypes.c_float), ("cg_tol", ctypes.c_float), ("cg_max_iter", ctypes.c_int32)]
+                ("eps", ctypes.c_float), ("cg_tol", ctypes.c_float), ("cg_max_iter", ctypes.c_int32), ("solver", ctypes.c_int32)]
 
 
 class _Grid(ctypes.Structure):
@@ -83,6 +83,7 @@ def load_library():
     lib.dm_shape_params_default.argtypes = [ctypes.POINTER(ShapeParams)]
     lib.dm_shape_state_create.argtypes = [vp, ctypes.POINTER(ShapeParams), ctypes.POINTER(vp)]
     lib.dm_shape_precondition.argtypes = [vp, vp, fp, fp]
+    lib.dm_shape_last_cg_iterations.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_int32)]
     lib.dm_shape_step.argtypes = [vp, vp, fp, fp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]
     lib.dm_shape_state_destroy.argtypes = [vp]
     lib.dm_shape_state_destroy.restype = None
@@ -269,7 +270,7 @@ class Plan:
 
     def shape_state(self, **params):
         """A ShapeState (dm_shape_state) of this plan; keyword arguments override dm_shape_params' defaults
-        (lr, lambda_, beta1, beta2, eps, cg_tol, cg_max_iter)."""
+        (lr, lambda_, beta1, beta2, eps, cg_tol, cg_max_iter, solver)."""
         return ShapeState(self, **params)
 
     def close(self):
@@ -310,6 +311,12 @@ class ShapeState:
         o = p._f32(out, p.n_vertices * 3, "out")
         _check(self._lib.dm_shape_precondition(p._h, self._h, gg.data_ptr(), o.data_ptr()), "dm_shape_precondition")
         return out
+
+    def last_cg_iterations(self):
+        """Iterations of the two solves of the last precondition / step ((-1, -1) for the multi-launch solve)."""
+        out = (ctypes.c_int32 * 2)()
+        _check(self._lib.dm_shape_last_cg_iterations(self._plan._h, self._h, out), "dm_shape_last_cg_iterations")
+        return int(out[0]), int(out[1])
 
     def step(self, vertices, target, psf_cov, return_loss: bool = False):
         """One step; ``vertices`` is updated in place.  With ``return_loss`` returns Phi_1 before the step (synchronises)."""

@@ -967,6 +967,8 @@ struct dm_shape_state {
     double *part_a = nullptr, *part_b = nullptr;
     DmCgScalars* cg_sc = nullptr;    // [2]: the scalars of the current and of the next iteration
     int cg_iter_bound = 0;           // iterations after which CG has converged to cg_tol whatever the right-hand side
+    int coop_blocks = 0;             // > 0: blocks of the persistent (cooperative) solve; 0: the multi-launch solve
+    int* cg_iters = nullptr;         // [2] device: iterations the two solves of the last preconditioning took (persistent solve)
     double *mom = nullptr, *amax_part = nullptr, *s_next = nullptr;
     DmAdamScalars* adam = nullptr;
     float *image = nullptr, *cot = nullptr, *grad = nullptr;
@@ -977,9 +979,22 @@ namespace {
 
 // x = M^-1 b, M = I + lambda L, for the three columns of b ([n][3], fp32 or fp64), by conjugate gradients on the device
 template <typename TB>
-int shape_cg_solve(dm_plan* p, dm_shape_state* st, const TB* b_dev, double* x_dev)
+int shape_cg_solve(dm_plan* p, dm_shape_state* st, const TB* b_dev, double* x_dev, int which)
 {
     const int n = p->n_vertices, nb = st->n_blocks;
+    if (st->coop_blocks > 0) {
+        // one persistent kernel: grid barriers instead of launches, stops at convergence
+        int n_ = n, max_iter = st->prm.cg_max_iter;
+        double lambda = (double)st->prm.lambda, tol2_ = (double)st->prm.cg_tol * (double)st->prm.cg_tol;
+        int* iters = st->cg_iters + which;
+        void* args[] = {(void*)&st->adj_off, (void*)&st->adj_idx, (void*)&n_, (void*)&lambda, (void*)&b_dev, (void*)&x_dev,
+                        (void*)&st->cg_r, (void*)&st->cg_p, (void*)&st->cg_Ap, (void*)&st->part_a, (void*)&st->part_b,
+                        (void*)&tol2_, (void*)&max_iter, (void*)&iters};
+        if (cudaLaunchCooperativeKernel((const void*)dm_k_cg_persistent<TB>, dim3((unsigned)st->coop_blocks), dim3(DM_SH_THREADS),
+                                        args, 0, p->stream) != cudaSuccess)
+            return DM_ERR_CUDA;
+        return check_launch(p, 1);
+    }
     dm_k_cg_init<TB><<<nb, DM_SH_THREADS, 0, p->stream>>>(b_dev, n, x_dev, st->cg_r, st->cg_p, st->part_a);
     dm_k_cg_init_final<<<1, DM_SH_THREADS, 0, p->stream>>>(st->part_a, nb, st->cg_sc);
     int rc = check_launch(p, 2);
@@ -1000,9 +1015,9 @@ int shape_cg_solve(dm_plan* p, dm_shape_state* st, const TB* b_dev, double* x_de
 // out = (I + lambda L)^-2 g: two solves (reading R27); the result stays in st->cg_x (fp64)
 int shape_precondition(dm_plan* p, dm_shape_state* st, const float* g_dev)
 {
-    int rc = shape_cg_solve<float>(p, st, g_dev, st->cg_y);
+    int rc = shape_cg_solve<float>(p, st, g_dev, st->cg_y, 0);
     if (rc) return rc;
-    return shape_cg_solve<double>(p, st, st->cg_y, st->cg_x);
+    return shape_cg_solve<double>(p, st, st->cg_y, st->cg_x, 1);
 }
 
 }  // namespace
@@ -1019,6 +1034,7 @@ int dm_shape_params_default(dm_shape_params* out)
     out->eps = 1e-8f;
     out->cg_tol = 1e-7f;
     out->cg_max_iter = 400;
+    out->solver = 0;
     return DM_OK;
 }
 
@@ -1031,7 +1047,7 @@ int dm_shape_state_create(dm_plan* p, const dm_shape_params* params, dm_shape_st
     dm_shape_params_default(&prm);
     if (params) prm = *params;
     if (!(prm.lr > 0.f) || !(prm.lambda >= 0.f) || !(prm.beta1 >= 0.f && prm.beta1 < 1.f) || !(prm.beta2 >= 0.f && prm.beta2 < 1.f) ||
-        !(prm.eps >= 0.f) || !(prm.cg_tol > 0.f) || prm.cg_max_iter < 1 || !std::isfinite(prm.lr) || !std::isfinite(prm.lambda))
+        !(prm.eps >= 0.f) || !(prm.cg_tol > 0.f) || prm.cg_max_iter < 1 || (prm.solver != 0 && prm.solver != 1) || !std::isfinite(prm.lr) || !std::isfinite(prm.lambda))
         return DM_ERR_INVALID_ARG;
     dm_shape_state* st = new (std::nothrow) dm_shape_state();
     if (!st) return DM_ERR_ALLOC;
@@ -1081,7 +1097,7 @@ int dm_shape_state_create(dm_plan* p, const dm_shape_params* params, dm_shape_st
             cudaMalloc(&st->cg_r, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->cg_p, n3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->cg_Ap, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->part_a, nb3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->part_b, nb3 * sizeof(double)) != cudaSuccess ||
-            cudaMalloc(&st->cg_sc, 2 * sizeof(DmCgScalars)) != cudaSuccess || cudaMalloc(&st->mom, n3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->cg_sc, 2 * sizeof(DmCgScalars)) != cudaSuccess || cudaMalloc(&st->cg_iters, 2 * sizeof(int)) != cudaSuccess || cudaMalloc(&st->mom, n3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->amax_part, DM_SH_LOSS_BLOCKS * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->s_next, sizeof(double)) != cudaSuccess || cudaMalloc(&st->adam, sizeof(DmAdamScalars)) != cudaSuccess ||
             cudaMalloc(&st->image, nvox * sizeof(float)) != cudaSuccess || cudaMalloc(&st->cot, nvox * sizeof(float)) != cudaSuccess ||
@@ -1093,7 +1109,22 @@ int dm_shape_state_create(dm_plan* p, const dm_shape_params* params, dm_shape_st
                                  cudaSuccess) ||
             cudaMemsetAsync(st->mom, 0, n3 * sizeof(double), p->stream) != cudaSuccess ||
             cudaMemsetAsync(st->adam, 0, sizeof(DmAdamScalars), p->stream) != cudaSuccess ||
+            cudaMemsetAsync(st->cg_iters, 0, 2 * sizeof(int), p->stream) != cudaSuccess ||
             cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
+        // the persistent solve needs every block resident at once (cooperative launch); blocks stride over the vertex tiles
+        {
+            int dev = 0, coop = 0, per_sm = 0;
+            if (prm.solver == 0 && cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess &&
+                coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, dm_k_cg_persistent<double>, DM_SH_THREADS, 0) == cudaSuccess &&
+                per_sm > 0) {
+                int per_sm_f = 0;
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_f, dm_k_cg_persistent<float>, DM_SH_THREADS, 0);
+                per_sm = std::min(per_sm, per_sm_f);
+                // a vertex tile per block when they all fit; otherwise a grid that fills the machine once
+                st->coop_blocks = std::min(st->n_blocks, per_sm * p->n_sm);
+            }
+            cudaGetLastError();
+        }
     } while (0);
     if (rc != DM_OK) {
         dm_shape_state_destroy(st);
@@ -1112,6 +1143,20 @@ int dm_shape_precondition(dm_plan* p, dm_shape_state* st, const float* g_dev, fl
     const int n3 = p->n_vertices * 3;
     dm_k_f64_to_f32<<<(n3 + 255) / 256, 256, 0, p->stream>>>(st->cg_x, n3, out_dev);
     return check_launch(p);
+}
+
+int dm_shape_last_cg_iterations(dm_plan* p, dm_shape_state* st, int32_t iters[2])
+{
+    if (!p || !st || st->plan != p || !iters) return DM_ERR_INVALID_ARG;
+    iters[0] = iters[1] = -1;
+    if (st->coop_blocks <= 0) return DM_OK;   // the multi-launch solve keeps no count
+    int h[2] = {0, 0};
+    if (cudaMemcpyAsync(h, st->cg_iters, sizeof(h), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+        cudaStreamSynchronize(p->stream) != cudaSuccess)
+        return DM_ERR_CUDA;
+    iters[0] = h[0];
+    iters[1] = h[1];
+    return DM_OK;
 }
 
 int dm_shape_step(dm_plan* p, dm_shape_state* st, float* vertices_dev, const float* target_dev, const float* psf_cov_host,
@@ -1160,6 +1205,7 @@ void dm_shape_state_destroy(dm_shape_state* st)
     cudaFree(st->part_a);
     cudaFree(st->part_b);
     cudaFree(st->cg_sc);
+    cudaFree(st->cg_iters);
     cudaFree(st->mom);
     cudaFree(st->amax_part);
     cudaFree(st->s_next);

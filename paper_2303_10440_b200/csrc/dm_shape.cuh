@@ -9,8 +9,9 @@
 // symmetric positive definite with condition number <= 1 + 2 lambda max_degree (about 700 for lambda = 50), the three
 // coordinate columns are solved at once with their own step lengths, vectors and dot products are fp64 (the work is
 // O(n_V) per iteration, nothing next to the mesh FT), and every reduction is a fixed-order two-stage tree, so the step is
-// bitwise reproducible.  One iteration = three small launches (the two dot products are grid-wide); a device flag turns the
-// remaining launches of a converged solve into no-ops, so the host never synchronises.
+// bitwise reproducible.  The solve is one persistent cooperative kernel (three grid barriers per iteration, it stops at
+// convergence) when every block fits on the device at once, else three small launches per iteration with a device flag that
+// turns the launches of a converged solve into no-ops; either way the host never synchronises.
 // AdamUniform (reading R28): Adam whose second moment is one scalar per step, the largest squared gradient entry.
 #pragma once
 #include <cuda_runtime.h>
@@ -251,4 +252,108 @@ __global__ void dm_k_f64_to_f32(const double* __restrict__ a, int n, float* __re
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) out[i] = (float)a[i];
+}
+
+// ---- the same conjugate-gradient solve as ONE persistent kernel (cooperative launch, grid-wide barriers) ----------------
+// Used when every block of the solve can be resident at once (always, up to ~3e5 vertices): the three launches per iteration
+// become three grid barriers, and the kernel STOPS at convergence instead of queueing no-op launches.  The arithmetic and
+// the order of every sum are those of the multi-launch kernels above (block partials in block order, every block adds them
+// alike), with the vertices of a block being the tiles blockIdx.x, blockIdx.x + gridDim.x, ...
+#include <cooperative_groups.h>
+
+// fixed-order block sum of three doubles per thread; every thread gets the results
+__device__ __forceinline__ void dm_sh_block_sum3(double v[3], double (*sh)[DM_SH_THREADS])
+{
+    __syncthreads();
+#pragma unroll
+    for (int c = 0; c < 3; ++c) sh[c][threadIdx.x] = v[c];
+    __syncthreads();
+    for (int s = DM_SH_THREADS / 2; s > 0; s >>= 1) {
+        if ((int)threadIdx.x < s)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) sh[c][threadIdx.x] += sh[c][threadIdx.x + s];
+        __syncthreads();
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) v[c] = sh[c][0];
+}
+// block partials out, grid barrier, total of all blocks' partials (the same on every block)
+__device__ __forceinline__ void dm_sh_grid_sum3(double v[3], double* __restrict__ part, double (*sh)[DM_SH_THREADS])
+{
+    dm_sh_block_sum3(v, sh);
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) part[3 * (size_t)blockIdx.x + c] = v[c];
+    cooperative_groups::this_grid().sync();
+    double a[3] = {0.0, 0.0, 0.0};
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += DM_SH_THREADS)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) a[c] += part[3 * (size_t)i + c];
+    dm_sh_block_sum3(a, sh);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) v[c] = a[c];
+}
+
+template <typename TB>
+__global__ void __launch_bounds__(DM_SH_THREADS)
+dm_k_cg_persistent(const int32_t* __restrict__ adj_off, const int32_t* __restrict__ adj_idx, int n, double lambda,
+                   const TB* __restrict__ b, double* __restrict__ x, double* __restrict__ r, double* __restrict__ p,
+                   double* __restrict__ Ap, double* __restrict__ part_a, double* __restrict__ part_b, double tol2, int max_iter,
+                   int* __restrict__ iters_out)
+{
+    __shared__ double sh[3][DM_SH_THREADS];
+    const int stride = (int)gridDim.x * DM_SH_THREADS;
+    const int i0 = (int)blockIdx.x * DM_SH_THREADS + (int)threadIdx.x;
+    double rr[3] = {0.0, 0.0, 0.0}, bb[3];
+    for (int i = i0; i < n; i += stride)
+        for (int c = 0; c < 3; ++c) {
+            const double v = (double)b[3 * (size_t)i + c];
+            x[3 * (size_t)i + c] = 0.0;
+            r[3 * (size_t)i + c] = v;
+            p[3 * (size_t)i + c] = v;
+            rr[c] += v * v;
+        }
+    dm_sh_grid_sum3(rr, part_a, sh);
+    for (int c = 0; c < 3; ++c) bb[c] = rr[c];
+    int it = 0;
+    for (; it < max_iter; ++it) {
+        if (rr[0] <= tol2 * bb[0] && rr[1] <= tol2 * bb[1] && rr[2] <= tol2 * bb[2]) break;   // the same on every block
+        double pAp[3] = {0.0, 0.0, 0.0};
+        for (int i = i0; i < n; i += stride) {
+            const int jb = adj_off[i], je = adj_off[i + 1];
+            double s[3] = {0.0, 0.0, 0.0};
+            for (int j = jb; j < je; ++j) {
+                const size_t q = 3 * (size_t)adj_idx[j];
+                s[0] += p[q], s[1] += p[q + 1], s[2] += p[q + 2];
+            }
+            const double deg = (double)(je - jb);
+            for (int c = 0; c < 3; ++c) {
+                const double pi = p[3 * (size_t)i + c];
+                const double a = pi + lambda * (deg * pi - s[c]);
+                Ap[3 * (size_t)i + c] = a;
+                pAp[c] += pi * a;
+            }
+        }
+        dm_sh_grid_sum3(pAp, part_b, sh);
+        double rn[3] = {0.0, 0.0, 0.0};
+        for (int i = i0; i < n; i += stride)
+            for (int c = 0; c < 3; ++c) {
+                const double alpha = pAp[c] > 0.0 ? rr[c] / pAp[c] : 0.0;
+                const size_t q = 3 * (size_t)i + c;
+                x[q] += alpha * p[q];
+                const double rv = r[q] - alpha * Ap[q];
+                r[q] = rv;
+                rn[c] += rv * rv;
+            }
+        dm_sh_grid_sum3(rn, part_a, sh);
+        for (int i = i0; i < n; i += stride)
+            for (int c = 0; c < 3; ++c) {
+                const double beta = rr[c] > 0.0 ? rn[c] / rr[c] : 0.0;
+                const size_t q = 3 * (size_t)i + c;
+                p[q] = r[q] + beta * p[q];
+            }
+        for (int c = 0; c < 3; ++c) rr[c] = rn[c];
+        cooperative_groups::this_grid().sync();   // p is complete before the next product reads the neighbours
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0 && iters_out) *iters_out = it;
 }

@@ -40,6 +40,15 @@ def test_preconditioner_against_dense_solves(dm, cfg, sub):
         assert err <= 1e-5
         out2 = st.precondition(torch.as_tensor(g, device="cuda")).cpu().numpy()
         assert np.array_equal(out, out2)                     # fixed-order reductions: bitwise reproducible
+        it = st.last_cg_iterations()
+        print(f"   CG iterations of the two solves: {it}")
+        assert all(0 <= i <= 300 for i in it) and (lam > 0 or it == (1, 1) or it == (0, 0) or max(it) <= 1)
+        # the multi-launch form of the same solve (used when a mesh does not fit one resident grid): same bits
+        st2 = plan.shape_state(lambda_=lam, solver=1)
+        out3 = st2.precondition(torch.as_tensor(g, device="cuda")).cpu().numpy()
+        assert st2.last_cg_iterations() == (-1, -1)
+        assert np.array_equal(out, out3)
+        st2.close()
         st.close()
     plan.close()
 
