@@ -991,9 +991,12 @@ int shape_cg_solve(dm_plan* p, dm_shape_state* st, const TB* b_dev, double* x_de
                         (void*)&st->cg_r, (void*)&st->cg_p, (void*)&st->cg_Ap, (void*)&st->part_a, (void*)&st->part_b,
                         (void*)&tol2_, (void*)&max_iter, (void*)&iters};
         if (cudaLaunchCooperativeKernel((const void*)dm_k_cg_persistent<TB>, dim3((unsigned)st->coop_blocks), dim3(DM_SH_THREADS),
-                                        args, 0, p->stream) != cudaSuccess)
-            return DM_ERR_CUDA;
-        return check_launch(p, 1);
+                                        args, 0, p->stream) == cudaSuccess)
+            return check_launch(p, 1);
+        // the device refused the cooperative launch (e.g. it cannot make the whole grid resident right now): the same solve
+        // as separate launches, from now on
+        cudaGetLastError();
+        st->coop_blocks = 0;
     }
     dm_k_cg_init<TB><<<nb, DM_SH_THREADS, 0, p->stream>>>(b_dev, n, x_dev, st->cg_r, st->cg_p, st->part_a);
     dm_k_cg_init_final<<<1, DM_SH_THREADS, 0, p->stream>>>(st->part_a, nb, st->cg_sc);
