@@ -70,6 +70,13 @@ typedef enum dm_status {
 int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_vertices, int32_t n_faces,
                    const int32_t* faces_dev, void* cuda_stream);
 
+/* Move the plan to another CUDA stream: all later calls are ordered on it.  The caller orders the two streams (work already
+ * queued on the old stream is not waited for).  Use: capture a whole optimisation step in a CUDA graph -- create the plan,
+ * run every call of the step once (first calls allocate workspace, which cannot be captured), set the capturing stream,
+ * capture, and replay; the 10 000-step fits of PAPER.md:261 on small meshes are launch-bound otherwise.  Inside a capture
+ * nothing synchronises as long as dL_dpsf_cov_host / loss_host are NULL; dm_plan_stage_ms is meaningless for captured calls. */
+int dm_plan_set_stream(dm_plan* plan, void* cuda_stream);
+
 /* Restrict the mesh-FT calls of this plan to the x-slab [ix_begin, ix_end) of the stored spectrum
  * (array rows, not signed frequencies).  dm_mesh_ft_forward then writes only those rows of F and
  * dm_mesh_ft_backward sums only over them (a partial dL/dv that the caller all-reduces over slabs;

@@ -13,7 +13,7 @@ DM_OPT_REUSE_SPECTRUM = 5
 
 # every symbol include/deltamic.h declares
 _SYMBOLS = (
-    "dm_plan_create", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_mesh_ft_backward_with_spectrum", "dm_render",
+    "dm_plan_create", "dm_plan_set_stream", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_mesh_ft_backward_with_spectrum", "dm_render",
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
     "dm_plan_launch_count", "dm_plan_paths_used", "dm_plan_destroy", "dm_error_string", "dm_version",
     "dm_shape_params_default", "dm_shape_state_create", "dm_shape_precondition", "dm_shape_last_cg_iterations", "dm_shape_step", "dm_shape_state_destroy",
@@ -60,6 +60,7 @@ def load_library():
     vp, fp, ip = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p
     lib.dm_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(_Grid), ctypes.c_int, ctypes.c_int32,
                                    ctypes.c_int32, ip, vp]
+    lib.dm_plan_set_stream.argtypes = [vp, vp]
     lib.dm_plan_set_slab.argtypes = [vp, ctypes.c_int32, ctypes.c_int32]
     lib.dm_plan_set_option.argtypes = [vp, ctypes.c_int, ctypes.c_double]
     lib.dm_plan_set_face_weights.argtypes = [vp, fp]
@@ -170,6 +171,12 @@ class Plan:
         return self.n[0] * self.n[1] * (self.n[2] // 2 + 1)
 
     # -- the C ABI, one method per entry point ------------------------------------------------------------------
+    def set_stream(self, stream=None):
+        """Queue all later calls on ``stream`` (a torch.cuda.Stream; default: the current stream), e.g. the capturing
+        stream of ``torch.cuda.graph``."""
+        self.stream = self._torch.cuda.current_stream(self.device) if stream is None else stream
+        _check(self._lib.dm_plan_set_stream(self._h, self.stream.cuda_stream), "dm_plan_set_stream")
+
     def set_slab(self, ix_begin: int, ix_end: int):
         _check(self._lib.dm_plan_set_slab(self._h, int(ix_begin), int(ix_end)), "dm_plan_set_slab")
 

@@ -592,6 +592,16 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
     return DM_OK;
 }
 
+int dm_plan_set_stream(dm_plan* p, void* cuda_stream)
+{
+    if (!p) return DM_ERR_INVALID_ARG;
+    p->stream = (cudaStream_t)cuda_stream;
+    if (p->have_fft && (cufftSetStream(p->fft_xy, p->stream) != CUFFT_SUCCESS || cufftSetStream(p->fft_z, p->stream) != CUFFT_SUCCESS ||
+                        cufftSetStream(p->fft_r2c, p->stream) != CUFFT_SUCCESS))
+        return DM_ERR_CUFFT;
+    return DM_OK;
+}
+
 int dm_plan_set_slab(dm_plan* p, int32_t ix_begin, int32_t ix_end)
 {
     if (!p || ix_begin < 0 || ix_end > p->gd.nx || ix_begin >= ix_end) return DM_ERR_INVALID_ARG;

@@ -580,3 +580,51 @@ def test_maximum_grid_extents(dm, n):
     import torch
     with pytest.raises(dm.DeltamicError):                                # one voxel more is refused, not mis-computed
         dm.Plan((4098, 2, 2), (1 / 4098, 0.5, 0.5), (0, 0, 0), 1, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+
+
+def test_cuda_graph_capture_of_an_optimisation_step(dm):
+    """dm_plan_set_stream: forward + backward, and a whole shape-optimisation step (render, Phi_1, backward, the two
+    cooperative CG solves, AdamUniform), captured into CUDA graphs after one eager warm-up and replayed: same bits as the
+    eager calls, no synchronisation inside."""
+    import torch
+    w = build_workload(1)
+    plan, vd = _plan(dm, w, 0), _dev(w.vertices)
+    Gd = _dev(spectrum_cotangent(w))
+    F = torch.empty(w.spectrum_shape, dtype=torch.complex64, device="cuda")
+    dv = torch.empty((w.vertices.shape[0], 3), dtype=torch.float32, device="cuda")
+    plan.mesh_ft_forward(vd, out=F)
+    plan.mesh_ft_backward(vd, Gd, out=dv)                 # eager warm-up: allocates the workspace
+    F0, dv0 = F.clone(), dv.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        plan.set_stream()                                  # the capturing stream
+        plan.mesh_ft_forward(vd, out=F)
+        plan.mesh_ft_backward(vd, Gd, out=dv)
+    plan.set_stream()
+    F.zero_()
+    dv.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(F, F0) and torch.equal(dv, dv0)
+    # a shape step: three eager steps against one eager warm-up + two replays of the captured step
+    cov = w.psf_cov
+    target = plan.render(_dev(build_workload(2, subdiv_override=2, grid_override=w.n).vertices), cov).clone()
+    v_e = vd.clone()
+    st = plan.shape_state(lr=1e-3)
+    for _ in range(3):
+        st.step(v_e, target, cov)
+    st.close()
+    v_g = vd.clone()
+    st = plan.shape_state(lr=1e-3)
+    st.step(v_g, target, cov)
+    g2 = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g2):
+        plan.set_stream()
+        st.step(v_g, target, cov)
+    plan.set_stream()
+    g2.replay()                                            # (capturing records the step, it does not run it)
+    g2.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(v_g, v_e)
+    st.close()
+    plan.close()
