@@ -288,10 +288,9 @@ dm_k_forward_fast(const float4* __restrict__ rec, const int32_t* __restrict__ ch
                         const float ky = __fmul_rn(grid.kstep[1], (float)(nys0 + j));
                         const float p = dm_edge_gap(ky, q1.z, gp);            // x1 - x0
                         const float q = __fadd_rn(p, dm_edge_gap(ky, r1.z, gn));  // x2 - x0
-                        cf psi, d1, d2;
-                        dm_psi_robust<false>(p, q, psi, d1, d2);
-                        const cf E = dm_expmi_turns(dm_phase_turns(nx, nys0 + j, nz, __float_as_uint(r0.x),
-                                                                   __float_as_uint(r0.y), __float_as_uint(r0.z)));
+                        const cf psi = dm_psi_value_fast(p, q);
+                        const cf E = dm_expmi_turns_fast(dm_phase_turns(nx, nys0 + j, nz, __float_as_uint(r0.x),
+                                                                        __float_as_uint(r0.y), __float_as_uint(r0.z)));
                         const float sc = (MODE == 1) ? r2.x : fmaf(kx, r2.x, fmaf(ky, r2.y, kz * r2.z));
                         const cf g = cscale(cmul(E, psi), sc);
 #pragma unroll

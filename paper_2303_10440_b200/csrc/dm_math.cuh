@@ -211,6 +211,42 @@ __device__ __forceinline__ void dm_psi_far_uniform(float p, float q, cf& psi, cf
     dq.im = B ? dj.im : dk.im;
 }
 
+// psi(p,q) alone, any (p,q), with MUFU sines / cosines on arguments reduced to [-pi, pi] (abs. error ~5e-7) -- for the
+// flagged pairs of the fast forward kernel: each is one triangle's term among >= 10^2..10^5, needed to ~1e-5 of its own size
+// (DESIGN.md section 6), and the fast path's own phase seeds have the same accuracy.  Same two branches as dm_psi_robust.
+__device__ __forceinline__ cf dm_dd2_value_fast(float al, float be)
+{
+    const float m = 0.5f * (al + be), h = 0.5f * (al - be);
+    float s;
+    if (fabsf(h) < 0.5f) {
+        const float h2 = h * h;
+        s = fmaf(h2, fmaf(h2, fmaf(h2, fmaf(h2, fmaf(h2, -1.0f / 39916800.0f, 1.0f / 362880.0f), -1.0f / 5040.0f), 1.0f / 120.0f),
+                          -1.0f / 6.0f), 1.0f);
+    } else {
+        const float hr = fmaf(-6.283185307179586f, rintf(h * 0.15915494309189535f), h);
+        s = __sinf(hr) * dm_rcp_approx(h);
+    }
+    const float mr = fmaf(-6.283185307179586f, rintf(m * 0.15915494309189535f), m);
+    return {__cosf(mr) * s, -__sinf(mr) * s};
+}
+__device__ __forceinline__ cf dm_psi_value_fast(float p, float q)
+{
+    const float ap = fabsf(p), aq = fabsf(q), ar = fabsf(q - p);
+    if (fmaxf(fmaxf(ap, aq), ar) < DM_SERIES_RADIUS) {
+        cf psi, d1, d2;
+        dm_psi_series<false>(p, q, psi, d1, d2);
+        return psi;
+    }
+    // nodes x0 = 0, x1 = p, x2 = q; the farthest pair (x_i, x_k) decides the roles, x_j is the third node
+    const bool A = (aq >= ap && aq >= ar);   // pair (0,2): i=0, j=1, k=2
+    const bool B = !A && (ap >= ar);         // pair (0,1): i=0, j=2, k=1;  else pair (1,2): i=1, j=0, k=2
+    const float xi = (A || B) ? 0.0f : p;
+    const float xj = A ? p : (B ? q : 0.0f);
+    const float xk = B ? p : q;
+    const cf D1 = dm_dd2_value_fast(xi, xj), D2 = dm_dd2_value_fast(xj, xk);
+    return cscale(cmul_i(csub(D1, D2)), dm_rcp_approx(xi - xk));
+}
+
 // psi(p,q) and its partials, any (p,q).  Robust ("slow") path.
 template <bool GRAD>
 __device__ __forceinline__ void dm_psi_robust(float p, float q, cf& psi, cf& dp, cf& dq)
