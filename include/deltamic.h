@@ -39,7 +39,7 @@ extern "C" {
 typedef struct dm_plan dm_plan; /* opaque */
 
 typedef struct dm_grid {
-    int32_t n[3];       /* voxels (x, y, z); the rfft half axis is z; n[2] must be even        */
+    int32_t n[3];       /* voxels (x, y, z), 1..4096 each; the rfft half axis is z; n[2] must be even */
     float   spacing[3]; /* voxel size per axis; box length L_a = n[a] * spacing[a]             */
     float   origin[3];  /* sample point of voxel (0,0,0) (its centre), reading R11             */
 } dm_grid;
