@@ -31,10 +31,10 @@
 // kernel has no limit on N_z.
 //
 // Near-degenerate pairs (reading R4).  The derivative coefficients grow like 1/(gap^2 gap'), so a pair
-// with  m1^2 m2 <= tau_b  (m1 <= m2 the two smallest |gaps|)  is excluded from the fast sums (its reciprocal is forced to
-// 0) and flagged in a per-thread bit mask.  After each chunk of 32 frequencies the lanes' flag WORDS are appended, in lane
-// order (one ballot and one 16-byte store per lane), to a ring buffer the WARP keeps in shared memory ACROSS chunks and
-// rows; whenever the buffer holds 32 pairs the warp evaluates them, one pair per lane whatever its owner (the series branch
+// with  m1^2 m2 <= tau_b  (m1 <= m2 the two smallest |gaps|)  is excluded from the fast sums (it accumulates nothing;
+// its reciprocal may be inf) and flagged in a per-thread bit mask.  After each chunk of 32 frequencies the lanes' flag
+// WORDS are appended, in lane order (one ballot and one 16-byte store per lane), to a ring buffer the WARP keeps in shared
+// memory ACROSS chunks and rows; whenever the buffer holds 32 pairs the warp evaluates them, one pair per lane whatever its owner (the series branch
 // where all gaps are small, the branch-free far-pair variant otherwise) -- always a full round, the remainder waits for the
 // next chunk.  Pair e of a round is found from a prefix sum of the words' bit counts, one warp reduce-or and an n-th-set-bit
 // select.  A segmented warp scan sums the results of one (row, owner) run, and the run's last lane hands them to the owner
