@@ -476,7 +476,7 @@ def run_ours(args):
         for c in [int(x) for x in args.extra_cfgs.split(",") if x.strip()]:
             if c == w.cfg or world > 1:
                 continue
-            wc, f_ms, b_ms, k_ms = time_config(dm, c, 1, 2 if c < 5 else 1)
+            wc, f_ms, b_ms, k_ms = time_config(dm, c, 3 if c <= 2 else 1, 10 if c <= 2 else (2 if c < 5 else 1))
             pc = float(wc.pairs)
             extra[f"cfg{c}"] = {
                 "mode": "surface" if wc.mode else "volume", "pairs_per_pass": pc, "fwd_ms": f_ms, "bwd_ms": b_ms,
@@ -535,7 +535,7 @@ def main():
     ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"],
                     help="replicas (default): every rank its own problem, weak scaling, no data-path collective; slab: ONE problem "
                          "sharded by x-slab of the stored spectrum (all-gather of F, all-reduce of dL/dv), strong scaling")
-    ap.add_argument("--extra-cfgs", default="3,5", help="other BASELINE.json configs timed (N=1 only) for the extra roofline "
+    ap.add_argument("--extra-cfgs", default="1,2,3,5", help="other BASELINE.json configs timed (N=1 only) for the extra roofline "
                     "entries; '' switches them off")
     ap.add_argument("--x-slab", default="", help="a:b -- profiling aid (ncu counters overflow on the 0.4 s full-grid launch): run "
                     "forward/backward on rows [a,b) of the spectrum only and print a short line that is NOT a bench result")
