@@ -87,7 +87,16 @@ int dm_plan_set_slab(dm_plan* plan, int32_t ix_begin, int32_t ix_end);
  * concentration).  weights_dev = device float32 [n_faces], copied here (the caller may free it); every triangle term of
  * F, and so of the gradients, is multiplied by its face's weight: DM_SURFACE sum_T w_T int_T e^{-ik.x} dS, DM_VOLUME
  * (i/|k|^2) sum_T w_T (k.m_T) f_T (closed components with one weight each are regions of that density; negative weights
- * carve holes).  F(0) is the weighted area / volume.  NULL switches the weights off (all 1, the default). */
+ * carve holes).  F(0) is the weighted area / volume.  NULL switches the weights off (all 1, the default).
+ * Accuracy.  The tolerance of the unweighted path, max|dF| <= 1e-4 |F(0)|, carries over to weights
+ * of ONE sign that, in DM_VOLUME, are constant on every connected component of the mesh (regions of different density):
+ * those keep the fast kernels.  Any other weight set -- mixed signs (F(0) cancels and is no longer the scale of the
+ * spectrum), or weights that vary inside a component in DM_VOLUME -- is evaluated pair by pair through the robust
+ * series / far-pair branches (several times slower; dm_plan_paths_used reports it), and its tolerance is stated against
+ * the scale of the same mesh with weights |w_T|:  max|dF| <= 1e-4 S_w,  S_w = sum_T |w_T| A_T  (DM_SURFACE)  or
+ * sum_T |w_T| A_T L_max / (2 pi)  (DM_VOLUME; A_T L_max / (2 pi) bounds a triangle's term at the lowest non-zero
+ * frequency).  The call reads the weights back to classify them, so it SYNCHRONISES the stream.  Non-finite weights
+ * return DM_ERR_INVALID_ARG. */
 int dm_plan_set_face_weights(dm_plan* plan, const float* weights_dev);
 
 /* Narrow band ("evaluate the FT only where the PSF spectrum is above 1 % of its maximum").
