@@ -13,7 +13,8 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2303_10440_b200.sharding import allgather_spectrum_slabs, allreduce_vertex_gradient, slab_bounds
+from paper_2303_10440_b200.sharding import (allgather_spectrum_slabs, allreduce_vertex_gradient, sharded_mesh_ft_backward,
+                                            sharded_mesh_ft_forward, slab_bounds)
 
 
 def test_slab_bounds_tile_the_grid():
@@ -39,6 +40,43 @@ def _free_port():
     p = s.getsockname()[1]
     s.close()
     return p
+
+
+class _OraclePlan:
+    """Stands in for paper_2303_10440_b200.Plan on CPU (same attributes and calls as sharding.py uses): the slab's rows are
+    evaluated by the oracle instead of the CUDA kernels.  What is under test is the host logic of the sharded calls."""
+
+    def __init__(self, w, mode):
+        self.w, self.mode = w, mode
+        self.n = w.n
+        self.spectrum_shape = w.spectrum_shape
+        self.n_vertices = w.vertices.shape[0]
+        self.device = torch.device("cpu")
+        self.slab = (0, w.n[0])
+        self.calls = []
+
+    def set_slab(self, b, e):
+        self.slab = (b, e)
+        self.calls.append(("slab", b, e))
+
+    def _idx(self):
+        nx, ny, nz = self.w.n
+        nzh = nz // 2 + 1
+        return np.arange(self.slab[0] * ny * nzh, self.slab[1] * ny * nzh, dtype=np.int64)
+
+    def mesh_ft_forward(self, vertices, out=None):
+        import oracle
+        idx = self._idx()
+        F = oracle.mesh_ft_forward_grid(vertices.numpy(), self.w.faces, self.w.n, self.w.spacing, self.mode, flat_indices=idx)
+        out.view(-1)[torch.as_tensor(idx)] = torch.as_tensor(F).to(out.dtype)
+        return out
+
+    def mesh_ft_backward(self, vertices, dL_dF):
+        import oracle
+        idx = self._idx()
+        G = dL_dF.reshape(-1).numpy()[idx].astype(np.complex128)
+        dv = oracle.mesh_ft_backward_grid(vertices.numpy(), self.w.faces, self.w.n, self.w.spacing, self.mode, G, flat_indices=idx)
+        return torch.as_tensor(np.asarray(dv, dtype=np.float32))
 
 
 def _worker(rank, world, port, out_dir):
@@ -72,6 +110,14 @@ def _worker(rank, world, port, out_dir):
             Fg[b:e] = torch.as_tensor(Fslab).reshape(e - b, ny, nzh)
             allgather_spectrum_slabs(Fg)
             np.save(os.path.join(out_dir, f"Fg_{mode}_{rank}.npy"), Fg.numpy())
+            # ... and the two sharded calls themselves, with the oracle standing in for the kernels
+            plan = _OraclePlan(w, mode)
+            vt = torch.as_tensor(w.vertices)
+            Fs2 = sharded_mesh_ft_forward(plan, vt, out=torch.zeros(w.spectrum_shape, dtype=torch.complex64))
+            dv2 = sharded_mesh_ft_backward(plan, vt, torch.as_tensor(G.astype(np.complex64)))
+            assert plan.slab == (0, nx)                                     # the plan is handed back on the whole grid
+            np.save(os.path.join(out_dir, f"Fs2_{mode}_{rank}.npy"), Fs2.numpy())
+            np.save(os.path.join(out_dir, f"dv2_{mode}_{rank}.npy"), dv2.numpy())
             np.save(os.path.join(out_dir, f"dv_{mode}_{rank}.npy"), dv.numpy())
             np.save(os.path.join(out_dir, f"F_{mode}_{rank}.npy"), torch.view_as_complex(Fr).numpy())
     finally:
@@ -97,3 +143,7 @@ def test_sharded_backward_allreduce_matches_whole_grid(world, tmp_path):
             assert np.abs(F - Fref).max() <= 1e-12 * abs(Fref[0])
             Fg = np.load(tmp_path / f"Fg_{mode}_{r}.npy").reshape(-1)
             assert np.isfinite(Fg).all() and np.abs(Fg - Fref).max() <= 1e-12 * abs(Fref[0])
+            Fs2 = np.load(tmp_path / f"Fs2_{mode}_{r}.npy").reshape(-1)
+            assert np.abs(Fs2 - Fref).max() <= 1e-6 * abs(Fref[0])          # complex64 storage
+            dv2 = np.load(tmp_path / f"dv2_{mode}_{r}.npy")
+            assert np.linalg.norm(dv2 - ref) <= 1e-6 * np.linalg.norm(ref)  # float32 partial gradients
