@@ -24,5 +24,7 @@ from ._binding import (  # noqa: F401
     version,
 )
 
-__all__ = ["Plan", "ShapeState", "ShapeParams", "DM_VOLUME", "DM_SURFACE", "DeltamicError", "load_library", "library_path", "exported_symbols",
+from .autograd import mesh_ft, render  # noqa: F401,E402
+
+__all__ = ["mesh_ft", "render", "Plan", "ShapeState", "ShapeParams", "DM_VOLUME", "DM_SURFACE", "DeltamicError", "load_library", "library_path", "exported_symbols",
            "version"]
