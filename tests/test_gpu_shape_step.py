@@ -102,3 +102,58 @@ def test_cfg4_ten_shape_steps_decrease_phi1(dm):
     assert losses[-1] < losses[0] and sum(b < a for a, b in zip(losses, losses[1:])) >= 8
     st.close()
     plan.close()
+
+
+def test_shape_fit_recovers_a_sphere_radius(dm):
+    """A miniature of the paper's reconstruction experiment on synthetic data: a sphere of radius 0.22
+    fitted, by repeated dm_shape_step calls, to the rendered image of a sphere of radius 0.30 -- the mean radius must move
+    most of the way, the mesh must stay round (the preconditioner keeps the update smooth) and Phi_1 must fall."""
+    import torch
+    from workloads import icosphere
+    v0, f = icosphere(2, 0.22)
+    vt, _ = icosphere(2, 0.30)
+    w = build_workload(1)                                  # grid and PSF of config 1 (32^3, sigma 1,1,2 voxels)
+    plan = dm.Plan(w.n, w.spacing, w.origin, 0, torch.as_tensor(f.astype(np.int32), device="cuda"), v0.shape[0])
+    target = plan.render(torch.as_tensor(vt.astype(np.float32), device="cuda"), w.psf_cov).clone()
+    vd = torch.as_tensor(v0.astype(np.float32), device="cuda").clone()
+    st = plan.shape_state(lr=2e-3)
+    losses = []
+    for it in range(80):
+        losses.append(st.step(vd, target, w.psf_cov, return_loss=(it % 10 == 0 or it == 79)))
+    r = torch.linalg.norm(vd, dim=1)
+    losses = [x for x in losses if x is not None]
+    print(f"sphere fit: mean radius 0.22 -> {float(r.mean()):.4f} (target 0.30), spread {float(r.std()):.2e}, "
+          f"Phi_1 {losses[0]:.3e} -> {losses[-1]:.3e}")
+    assert float(r.mean()) > 0.28 and float(r.std()) < 5e-3
+    assert losses[-1] < 0.1 * losses[0]
+    st.close()
+    plan.close()
+
+
+def test_psf_fit_with_adam_through_the_autograd_front_end(dm):
+    """A miniature of the paper's PSF step (phi_0 = ||u - m||^2, Adam [32] on Sigma): the three variances
+    of the PSF fitted to an image rendered with other variances, with torch.optim.Adam driving dm.render's gradient
+    w.r.t. the six PSF numbers."""
+    import torch
+    w = build_workload(1)
+    plan = dm.Plan(w.n, w.spacing, w.origin, 0, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    v = torch.as_tensor(w.vertices, device="cuda")
+    h = np.array(w.spacing)
+    cov_true = np.array([(1.6 * h[0]) ** 2, (1.2 * h[1]) ** 2, (2.4 * h[2]) ** 2, 0.0, 0.0, 0.0])
+    target = plan.render(v, cov_true).clone()
+    s = torch.tensor([1.0, 1.0, 1.0], dtype=torch.float64, requires_grad=True)      # sigma in voxels: cov = (s h)^2
+    opt = torch.optim.Adam([s], lr=0.05)
+    ht = torch.as_tensor(h)
+    first = last = None
+    for it in range(120):
+        opt.zero_grad()
+        cov = torch.cat([(s * ht) ** 2, torch.zeros(3, dtype=torch.float64)]).to(torch.float32)
+        loss = ((dm.render(plan, v, cov) - target) ** 2).sum()
+        loss.backward()
+        opt.step()
+        last = float(loss.detach())
+        first = last if first is None else first
+    got = s.detach().numpy()
+    print(f"PSF fit: sigma (voxels) 1,1,1 -> {got.round(3)} (target 1.6, 1.2, 2.4), phi_0 {first:.3e} -> {last:.3e}")
+    assert np.abs(got - np.array([1.6, 1.2, 2.4])).max() < 0.1 and last < 1e-2 * first
+    plan.close()
