@@ -57,7 +57,8 @@ typedef enum dm_status {
     DM_ERR_ALLOC       = -3, /* host or device allocation failed                                        */
     DM_ERR_CUDA        = -4, /* a CUDA runtime call or kernel launch failed                             */
     DM_ERR_CUFFT       = -5, /* a cuFFT call failed                                                     */
-    DM_ERR_UNSUPPORTED = -6  /* the requested feature is not built                                      */
+    DM_ERR_UNSUPPORTED = -6, /* the requested feature is not built                                      */
+    DM_ERR_TOO_LARGE   = -7  /* dm_mesh_ft_forward_noalloc: n_faces > DM_NOALLOC_MAX_FACES                      */
 } dm_status;
 
 /* Create a plan for one grid, mode and mesh topology.
@@ -249,6 +250,47 @@ int dm_shape_step(dm_plan* plan, dm_shape_state* state, float* vertices_dev, con
                   const float* psf_cov_host, double* loss_host);
 
 void dm_shape_state_destroy(dm_shape_state* state);
+
+/* ---- Forward mesh FT without a plan and without any memory allocation ----------------------------------------------------
+ * Who this is for.  Everything above goes through a plan, and a plan gets its workspace from cudaMalloc (at creation, and
+ * lazily on some first calls).  Some programs cannot afford that: a process that gave the whole GPU to one arena at start-up
+ * (a framework's caching allocator, a fixed memory budget per service) may find that a raw cudaMalloc fails or is forbidden
+ * by policy; a latency-bound loop cannot accept that cudaMalloc / cudaFree stall the device while they run; and code called
+ * from inside someone else's pipeline often has no say over when allocation is allowed.  Such callers hand in their own
+ * input and output buffers and call this function, which asks the CUDA runtime for no memory at all (no cudaMalloc, no
+ * cudaFree, no cuFFT or other allocating library routine, no host allocation).
+ *
+ * What it computes.  The same F as dm_mesh_ft_forward on a fresh plan of this grid and mode (whole grid, no narrow band, no
+ * face weights, no area normalisation; eq. 8-9, volume mode as above), with every (triangle, frequency)
+ * pair evaluated through the series / far-pair branches -- the kernels a plan runs under DM_OPT_FORWARD_PATH = 1.  It meets
+ * the same tolerance (max|dF| <= 1e-4 |F(0)|) but is several times slower than the plan's strip kernel: it is meant for
+ * small and medium meshes, not for the bench workloads.
+ *
+ * Where the scratch lives.  The triangle records (64 bytes per face) and the block sums of the k = 0 entry sit in a
+ * fixed array compiled into the library, DM_NOALLOC_MAX_FACES * 64 + 1024 bytes (4 MiB + 1 KiB).  Every GPU on which the
+ * library's kernels are loaded carries that array until the process exits, whether or not this function is ever called.
+ * n_faces > DM_NOALLOC_MAX_FACES returns DM_ERR_TOO_LARGE before anything is launched.
+ *
+ * Sharing.  There is one array per GPU and every call on that GPU uses it, from any thread and on any stream.  Two calls
+ * whose kernels can run at the same time on one GPU (different streams without an event between them, or two host
+ * threads) overwrite each other's records and both results are garbage: the caller serialises them.  Calls on one stream,
+ * or on different GPUs, are safe.  The array keeps whatever the previous call left in it; this function overwrites every
+ * byte it later reads, so no clearing is needed and a call never sees an earlier call's data.
+ *
+ * First call on a GPU.  The first call made while a given device is current looks up that device's address of the array
+ * (cudaGetSymbolAddress; this may also make the runtime load the library's kernels onto that GPU) and remembers it.  Make
+ * that first call during set-up, with the device you will use current, before any CUDA stream capture is begun.
+ *
+ *   grid          as in dm_plan_create (origin is not used by the mesh FT)
+ *   vertices_dev  device float32 [n_vertices*3]
+ *   faces_dev     device int32 [n_faces*3]; indices must lie inside the vertex array -- NOT checked here (checking needs a
+ *                 copy to the host), an out-of-range index reads out of bounds
+ *   F_dev         device complex64 [n_x*n_y*(n_z/2+1)], overwritten
+ *   cuda_stream   a cudaStream_t; NULL = the legacy default stream.  The call is asynchronous on it.
+ * Returns DM_OK, DM_ERR_INVALID_ARG, DM_ERR_TOO_LARGE or DM_ERR_CUDA. */
+#define DM_NOALLOC_MAX_FACES 65536
+int dm_mesh_ft_forward_noalloc(const dm_grid* grid, int mode, const float* vertices_dev, const int32_t* faces_dev,
+                               int32_t n_faces, float* F_dev, void* cuda_stream);
 
 const char* dm_error_string(int code);
 

@@ -21,10 +21,13 @@ from ._binding import (  # noqa: F401
     exported_symbols,
     library_path,
     load_library,
+    mesh_ft_forward_noalloc,
+    DM_NOALLOC_MAX_FACES,
+    DM_ERR_TOO_LARGE,
     version,
 )
 
 from .autograd import mesh_ft, render  # noqa: F401,E402
 
-__all__ = ["mesh_ft", "render", "Plan", "ShapeState", "ShapeParams", "DM_VOLUME", "DM_SURFACE", "DeltamicError", "load_library", "library_path", "exported_symbols",
+__all__ = ["mesh_ft", "render", "mesh_ft_forward_noalloc", "DM_NOALLOC_MAX_FACES", "DM_ERR_TOO_LARGE", "Plan", "ShapeState", "ShapeParams", "DM_VOLUME", "DM_SURFACE", "DeltamicError", "load_library", "library_path", "exported_symbols",
            "version"]

@@ -17,7 +17,10 @@ _SYMBOLS = (
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
     "dm_plan_launch_count", "dm_plan_paths_used", "dm_plan_destroy", "dm_error_string", "dm_version",
     "dm_shape_params_default", "dm_shape_state_create", "dm_shape_precondition", "dm_shape_last_cg_iterations", "dm_shape_step", "dm_shape_state_destroy",
+    "dm_mesh_ft_forward_noalloc",
 )
+DM_NOALLOC_MAX_FACES = 65536
+DM_ERR_TOO_LARGE = -7
 
 
 class DeltamicError(RuntimeError):
@@ -88,6 +91,7 @@ def load_library():
     lib.dm_shape_step.argtypes = [vp, vp, fp, fp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]
     lib.dm_shape_state_destroy.argtypes = [vp]
     lib.dm_shape_state_destroy.restype = None
+    lib.dm_mesh_ft_forward_noalloc.argtypes = [ctypes.POINTER(_Grid), ctypes.c_int, fp, ip, ctypes.c_int32, fp, vp]
     for name in _SYMBOLS:
         fn = getattr(lib, name)
         if name not in ("dm_plan_launch_count", "dm_plan_destroy", "dm_error_string", "dm_shape_state_destroy"):
@@ -117,6 +121,36 @@ def _cov(psf_cov):
     if len(vals) != 6:
         raise ValueError("psf_cov must hold 6 numbers: xx, yy, zz, xy, xz, yz")
     return (ctypes.c_float * 6)(*vals)
+
+
+def mesh_ft_forward_noalloc(n, spacing, mode: int, vertices, faces, out, stream=None):
+    """dm_mesh_ft_forward_noalloc: the forward mesh FT for callers that may not allocate device memory (a process whose
+    GPU memory is already committed to one arena, a loop that cannot take cudaMalloc's device-wide stall).  No plan; the
+    library's scratch is a fixed 4 MiB array inside libdeltamic.so, shared by every call on the GPU, so calls that could
+    overlap on one GPU must be serialised by the caller, and ``faces`` may hold at most DM_NOALLOC_MAX_FACES triangles
+    (DeltamicError with code DM_ERR_TOO_LARGE beyond that).  Nothing is allocated or converted here either: ``vertices``
+    (float32 [n_v, 3]), ``faces`` (int32 [n_f, 3]) and ``out`` (complex64 [n_x, n_y, n_z/2+1], overwritten and returned)
+    must already be contiguous CUDA tensors of those types.  Queued on ``stream`` (default: torch's current stream)."""
+    import torch
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2303_10440_b200 needs a CUDA device (no CPU fallback)")
+    lib = load_library()
+    n = tuple(int(v) for v in n)
+    for t, dt, name in ((vertices, torch.float32, "vertices"), (faces, torch.int32, "faces"), (out, torch.complex64, "out")):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dt and t.is_contiguous()):
+            raise ValueError(f"{name} must be a contiguous CUDA tensor of dtype {dt}")
+    if vertices.dim() != 2 or vertices.shape[1] != 3 or faces.dim() != 2 or faces.shape[1] != 3:
+        raise ValueError("vertices must be [n_v, 3] and faces [n_f, 3]")
+    if tuple(out.shape) != (n[0], n[1], n[2] // 2 + 1):
+        raise ValueError("out must have the rfft half-spectrum shape [n_x, n_y, n_z/2+1]")
+    grid = _Grid((ctypes.c_int32 * 3)(*n), (ctypes.c_float * 3)(*[float(v) for v in spacing]), (ctypes.c_float * 3)(0.0, 0.0, 0.0))
+    s = torch.cuda.current_stream(out.device) if stream is None else stream
+    with torch.cuda.device(out.device):
+        _check(lib.dm_mesh_ft_forward_noalloc(ctypes.byref(grid), int(mode), vertices.data_ptr(), faces.data_ptr(),
+                                              int(faces.shape[0]), out.data_ptr(), ctypes.c_void_p(s.cuda_stream)),
+               "dm_mesh_ft_forward_noalloc")
+    return out
 
 
 class Plan:

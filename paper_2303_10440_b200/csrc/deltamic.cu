@@ -8,6 +8,7 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <utility>
 #include <vector>
@@ -89,7 +90,8 @@ struct dm_plan {
 namespace {
 
 const char* kErr[] = {"ok", "invalid argument", "bad mesh (face index out of range)", "allocation failed",
-                      "CUDA error", "cuFFT error", "unsupported"};
+                      "CUDA error", "cuFFT error", "unsupported",
+                      "mesh too large for the fixed scratch of dm_mesh_ft_forward_noalloc"};
 
 inline size_t n_k_of(const dm_plan* p) { return (size_t)p->gd.nx * p->gd.ny * p->gd.nzh; }
 
@@ -400,7 +402,7 @@ int dm_version(void) { return DM_VERSION; }
 const char* dm_error_string(int code)
 {
     const int i = -code;
-    return (i >= 0 && i <= 6) ? kErr[i] : "unknown error";
+    return (i >= 0 && i <= 7) ? kErr[i] : "unknown error";
 }
 
 int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_vertices, int32_t n_faces,
@@ -1232,3 +1234,87 @@ void dm_shape_state_destroy(dm_shape_state* st)
 }
 
 }  // extern "C"
+
+// ---- dm_mesh_ft_forward_noalloc: forward mesh FT for callers that must not allocate (include/deltamic.h) -----------------
+//
+// The plan-based forward keeps its scratch (triangle records, block sums of the k = 0 entry) in cudaMalloc'ed workspace.
+// This variant keeps the same scratch in ONE array that is part of the library image: the driver places it in device
+// memory when the module is loaded on a GPU and releases it when the process exits, so the call itself never asks the
+// driver for memory.  Layout (bytes):  [0, 64 n_faces) triangle records of dm_k_geometry,
+// [DM_NA_REC_BYTES, +8 DM_DC_BLOCKS) block sums of dm_k_dc_partial, then one double for dm_k_dc_final's total.
+// All three regions are fully overwritten before they are read, so nothing has to start at zero.
+namespace {
+
+constexpr size_t DM_NA_REC_BYTES = (size_t)DM_NOALLOC_MAX_FACES * 4 * sizeof(float4);
+constexpr size_t DM_NA_SCRATCH_BYTES = DM_NA_REC_BYTES + 1024;
+static __device__ __align__(256) unsigned char dm_na_scratch[DM_NA_SCRATCH_BYTES];
+
+// `dm_na_scratch` in HOST code is only a handle for the runtime, not a device address.  The address differs from GPU
+// to GPU, so it is looked up once per device (with that device current) and remembered.
+constexpr int DM_NA_MAX_DEVICES = 64;
+void* g_na_ptr[DM_NA_MAX_DEVICES] = {};
+std::mutex g_na_mutex;
+
+int noalloc_scratch(unsigned char** out)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= DM_NA_MAX_DEVICES) return DM_ERR_CUDA;
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    if (!g_na_ptr[dev]) {
+        void* ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, dm_na_scratch) != cudaSuccess || !ptr) return DM_ERR_CUDA;
+        g_na_ptr[dev] = ptr;
+    }
+    *out = static_cast<unsigned char*>(g_na_ptr[dev]);
+    return DM_OK;
+}
+
+}  // namespace
+
+extern "C" int dm_mesh_ft_forward_noalloc(const dm_grid* grid, int mode, const float* vertices_dev, const int32_t* faces_dev,
+                                          int32_t n_faces, float* F_dev, void* cuda_stream)
+{
+    if (!grid || !vertices_dev || !faces_dev || !F_dev || n_faces <= 0 || (mode != DM_VOLUME && mode != DM_SURFACE))
+        return DM_ERR_INVALID_ARG;
+    for (int d = 0; d < 3; ++d)
+        if (grid->n[d] <= 0 || grid->n[d] > 4096 || !(grid->spacing[d] > 0.f) || !std::isfinite(grid->spacing[d]))
+            return DM_ERR_INVALID_ARG;
+    if (grid->n[2] % 2 != 0) return DM_ERR_INVALID_ARG;
+    if (n_faces > DM_NOALLOC_MAX_FACES) return DM_ERR_TOO_LARGE;   // the records would not fit the fixed array
+
+    unsigned char* scratch = nullptr;
+    int rc = noalloc_scratch(&scratch);   // first call on this device: looks the array's device address up
+    if (rc) return rc;
+    float4* rec = reinterpret_cast<float4*>(scratch);
+    double* dc_part = reinterpret_cast<double*>(scratch + DM_NA_REC_BYTES);
+    double* dc_total = dc_part + DM_DC_BLOCKS;
+
+    DmGridDev gd;
+    std::memset(&gd, 0, sizeof(gd));
+    gd.nx = grid->n[0];
+    gd.ny = grid->n[1];
+    gd.nz = grid->n[2];
+    gd.nzh = grid->n[2] / 2 + 1;
+    double lmax = 0.0;
+    for (int d = 0; d < 3; ++d) {
+        const double L = (double)grid->n[d] * (double)grid->spacing[d];
+        gd.kstep[d] = (float)(2.0 * M_PI / L);
+        gd.inv_len[d] = 1.0 / L;
+        lmax = std::max(lmax, L);
+    }
+    gd.band_lim = INFINITY;   // no narrow band, no face weights: the plain F of eq. 8-9
+    gd.nzb = gd.nzh;
+    gd.edge_fix = (float)(1073741824.0 / (lmax * lmax));
+    gd.inv_edge_norm = (float)(1.0 / (3.0 * (double)n_faces * (double)gd.edge_fix));
+
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    dm_k_geometry<<<(n_faces + 127) / 128, 128, 0, stream>>>(vertices_dev, faces_dev, n_faces, gd, rec);
+    if (cudaGetLastError() != cudaSuccess) return DM_ERR_CUDA;
+    const long long n_k = (long long)gd.nx * gd.ny * gd.nzh;
+    dm_k_forward_robust<<<(unsigned)((n_k + 127) / 128), 128, 0, stream>>>(rec, n_faces, gd, mode, 0, gd.nx, (float2*)F_dev);
+    if (cudaGetLastError() != cudaSuccess) return DM_ERR_CUDA;
+    dm_k_dc_partial<<<DM_DC_BLOCKS, 256, 0, stream>>>(vertices_dev, faces_dev, n_faces, mode, nullptr, dc_part);
+    if (cudaGetLastError() != cudaSuccess) return DM_ERR_CUDA;
+    dm_k_dc_final<<<1, DM_DC_BLOCKS, 0, stream>>>(dc_part, F_dev, dc_total);
+    return cudaGetLastError() == cudaSuccess ? DM_OK : DM_ERR_CUDA;
+}

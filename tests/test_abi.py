@@ -47,6 +47,24 @@ def test_host_only_entry_points(lib):
     lib.dm_plan_destroy(None)
 
 
+def test_noalloc_entry_point_validates_before_any_cuda_call(lib):
+    """dm_mesh_ft_forward_noalloc refuses bad arguments and meshes beyond its fixed scratch on the host, before it touches
+    the GPU (the pointers below are never dereferenced)."""
+    from paper_2303_10440_b200._binding import _Grid
+    import paper_2303_10440_b200 as dm
+    g = _Grid((ctypes.c_int32 * 3)(8, 8, 8), (ctypes.c_float * 3)(0.125, 0.125, 0.125), (ctypes.c_float * 3)(0, 0, 0))
+    fake = ctypes.c_void_p(256)
+    assert lib.dm_mesh_ft_forward_noalloc(None, 0, fake, fake, 1, fake, None) == -1
+    assert lib.dm_mesh_ft_forward_noalloc(ctypes.byref(g), 0, None, fake, 1, fake, None) == -1
+    assert lib.dm_mesh_ft_forward_noalloc(ctypes.byref(g), 2, fake, fake, 1, fake, None) == -1
+    assert lib.dm_mesh_ft_forward_noalloc(ctypes.byref(g), 0, fake, fake, 0, fake, None) == -1
+    assert lib.dm_mesh_ft_forward_noalloc(ctypes.byref(g), 0, fake, fake, dm.DM_NOALLOC_MAX_FACES + 1, fake, None) == dm.DM_ERR_TOO_LARGE
+    assert b"too large" in lib.dm_error_string(dm.DM_ERR_TOO_LARGE)
+    header = open(os.path.join(ROOT, "include", "deltamic.h")).read()
+    assert f"#define DM_NOALLOC_MAX_FACES {dm.DM_NOALLOC_MAX_FACES}" in header
+    assert "DM_ERR_TOO_LARGE   = -7" in header
+
+
 def test_product_path_has_no_oracle_or_cpu_fallback():
     """The package never imports oracle/ and refuses to run without CUDA."""
     import torch
