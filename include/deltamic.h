@@ -195,7 +195,10 @@ int64_t dm_plan_launch_count(const dm_plan* plan);
 
 /* Which kernels the LAST forward / backward mesh FT of this plan ran: paths[0] forward, paths[1] backward;
  * 0 = fast kernels, 1 = robust kernels (every pair through the series / far-pair branches: DM_OPT_*_PATH = 1, or a
- * weight set outside the fast kernels' validated regime), -1 = no such call yet.  Host-side bookkeeping, no sync. */
+ * weight set outside the fast kernels' validated regime), -1 = no such call yet.  Host-side bookkeeping, no sync.
+ * (The fast backward kernel indexes the (i_x, i_y) rows of one k-split with 15 bits; the plan always cuts the grid into
+ * enough splits for that -- csrc/dm_splits.h, at most 32768 rows each -- so grid or mesh size alone never selects the
+ * robust kernel.) */
 int dm_plan_paths_used(const dm_plan* plan, int32_t paths[2]);
 
 void dm_plan_destroy(dm_plan* plan);

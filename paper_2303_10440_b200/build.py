@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdeltamic.so")
 SOURCES = ["deltamic.cu"]
-HEADERS = ["dm_math.cuh", "dm_kernels.cuh", "dm_fast.cuh", "dm_bwd_fast.cuh", "dm_strips.h", "dm_patches.h", os.path.join("..", "..", "include", "deltamic.h")]
+HEADERS = ["dm_math.cuh", "dm_kernels.cuh", "dm_fast.cuh", "dm_bwd_fast.cuh", "dm_strips.h", "dm_patches.h", "dm_splits.h", "dm_shape.cuh", os.path.join("..", "..", "include", "deltamic.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

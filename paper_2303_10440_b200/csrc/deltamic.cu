@@ -17,6 +17,7 @@
 #include "dm_fast.cuh"
 #include "dm_bwd_fast.cuh"
 #include "dm_strips.h"
+#include "dm_splits.h"
 #include "dm_shape.cuh"
 
 #define DM_VERSION 100
@@ -122,21 +123,8 @@ void stage_reset(dm_plan* p)
 
 int backward_splits(const dm_plan* p, int* rows_per_split)
 {
-    // enough (triangle-block x k-split) CTAs to fill the machine (5 CTAs per SM) about 10 times over: short tail
-    const int n_rows = (p->ix_end - p->ix_begin) * p->gd.ny;
-    const int tri_blocks = (p->n_faces + 127) / 128;
-    int want = (p->n_sm * DM_BWD_SPLIT_TARGET + tri_blocks - 1) / tri_blocks;
-    if (p->band_on) want = std::max(want, std::min(p->n_split_max, 64));   // rows differ in cost under the narrow band:
-                                                                             // many small CTAs balance the load
-    // a CTA sets up its seed table and records once: give it at least ~512 frequencies per triangle
-    const int min_rows = (512 + p->gd.nzh - 1) / p->gd.nzh;
-    if (want > n_rows / min_rows) want = n_rows / min_rows;
-    if (want < 1) want = 1;
-    if (want > n_rows) want = n_rows;
-    if (want > p->n_split_max) want = p->n_split_max;
-    const int rps = (n_rows + want - 1) / want;
-    *rows_per_split = rps;
-    return (n_rows + rps - 1) / rps;
+    return dm_backward_splits((p->ix_end - p->ix_begin) * p->gd.ny, p->gd.nzh, p->n_faces, p->n_sm, DM_BWD_SPLIT_TARGET,
+                              p->band_on, p->n_split_max, rows_per_split);
 }
 
 int make_psf(const dm_plan* p, const float* cov, DmPsfDev* out)
@@ -284,7 +272,7 @@ int run_backward(dm_plan* p, const float* vertices_dev, const float* G_dev, floa
     const int seg = nzh <= 72 ? 8 : (nzh <= 144 ? 16 : 32);
     const int n_tab = std::min(DM_BF_NTAB_MAX, (nzh + seg - 1) / seg - 1);
     int rc;
-    const bool robust = p->bwd_path != 0 || p->weights_robust || rps > 32768;
+    const bool robust = p->bwd_path != 0 || p->weights_robust || rps > DM_SPLIT_MAX_ROWS;
     p->last_bwd_path = robust ? 1 : 0;
     if (!robust) {
         const DmPatchDev pt = {p->pt_face, p->pt_vid, p->pt_loc, p->pt_lanes};
@@ -505,15 +493,7 @@ int dm_plan_create(dm_plan** out, const dm_grid* grid, int mode, int32_t n_verti
         const size_t nk = n_k_of(p);
         // k-splits of the backward: a small mesh has few triangle blocks, so it needs many splits to fill the machine
         // (up to 48 CTAs per SM slot), within 64 M floats of partial sums
-        {
-            const long long tri_blocks = ((long long)n_faces + 127) / 128;
-            long long m = ((long long)p->n_sm * DM_BWD_SPLIT_TARGET + tri_blocks - 1) / tri_blocks;
-            m = std::min<long long>(m, (64LL << 20) / ((long long)DM_BWD_NSUM * n_faces));
-            p->n_split_max = (int)std::max<long long>(64, std::min<long long>(m, 4096));
-            // the fast kernel's queue entries hold a 15-bit row index inside the split
-            const long long rows = (long long)p->gd.nx * p->gd.ny;
-            p->n_split_max = (int)std::max<long long>(p->n_split_max, (rows + 32767) / 32768);
-        }
+        p->n_split_max = dm_backward_split_max(p->n_sm, DM_BWD_SPLIT_TARGET, DM_BWD_NSUM, n_faces, (long long)p->gd.nx * p->gd.ny);
         if (cudaMalloc(&p->faces, faces_h.size() * sizeof(int32_t)) != cudaSuccess ||
             cudaMalloc(&p->csr_off, off.size() * sizeof(int32_t)) != cudaSuccess ||
             cudaMalloc(&p->csr_corner, cor.size() * sizeof(int32_t)) != cudaSuccess ||

@@ -93,3 +93,44 @@ def test_strip_records_close_every_face_once_with_a_consistent_window(dumper, tm
         for i in range(lo, hi):
             assert vprev[i] == p1 and vret[i] == p2, (c, i)
             p2, p1 = p1, (vnew[i] if i < first_flush else -1)
+
+
+# ---- k-splits of the backward (dm_splits.h) -----------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def split_dumper(tmp_path_factory):
+    exe = tmp_path_factory.mktemp("host") / "dump_splits"
+    subprocess.run(["g++", "-O2", "-std=c++17", "-o", str(exe), os.path.join(HERE, "host", "dump_splits.cpp")], check=True)
+    return str(exe)
+
+
+def _splits(exe, nx, ny, nzh, n_faces, n_sm=148, band=0, slab=None):
+    args = [exe, str(nx), str(ny), str(nzh), str(n_faces), str(n_sm), str(band)]
+    if slab is not None:
+        args += [str(slab[0]), str(slab[1])]
+    out = subprocess.run(args, check=True, capture_output=True, text=True).stdout.split()
+    return tuple(int(x) for x in out)   # n_split_max, n_split, rows_per_split
+
+
+def test_backward_splits_never_outgrow_the_fast_kernels_row_index(split_dumper):
+    """A split holds at most 32768 rows (the fast backward kernel's 15-bit row index), whatever the mesh and grid: a huge
+    mesh (few splits wanted) on a wide grid used to get one split of nx*ny rows and fell back to the robust kernel."""
+    cases = [(4096, 64, 33, 4_000_000), (4096, 4096, 2, 5_000_000), (512, 512, 257, 3_600_000), (4096, 4096, 2, 320),
+             (128, 128, 65, 102_400), (256, 256, 129, 327_680), (32, 32, 17, 320), (2, 2, 2, 12)]
+    for nx, ny, nzh, n_faces in cases:
+        for band in (0, 1):
+            n_max, n_split, rps = _splits(split_dumper, nx, ny, nzh, n_faces, band=band)
+            n_rows = nx * ny
+            assert 1 <= n_split <= n_max, (nx, ny, nzh, n_faces)
+            assert rps <= 32768, (nx, ny, nzh, n_faces, rps)
+            assert (n_split - 1) * rps < n_rows <= n_split * rps       # the splits tile the rows, none is empty
+            assert n_max * 13 * n_faces <= max(64 * 13 * n_faces, (n_rows + 32767) // 32768 * 13 * n_faces, 64 << 20)
+    # the case of the report: ~4 M faces, 262144 rows -> 8 splits of 32768 rows rather than 1 of 262144
+    assert _splits(split_dumper, 4096, 64, 33, 4_000_000)[1:] == (8, 32768)
+    # x-slabs keep the bound too
+    assert _splits(split_dumper, 4096, 4096, 2, 4_000_000, slab=(0, 2048))[2] <= 32768
+
+
+def test_backward_splits_of_the_bench_configs_are_unchanged(split_dumper):
+    """The fix must not move the launch configuration bench.py times (cfg 4: 128^3, 102400 triangles; cfg 5: 256^3, 327680)."""
+    assert _splits(split_dumper, 128, 128, 65, 102_400) == (64, 36, 456)
+    assert _splits(split_dumper, 256, 256, 129, 327_680) == (64, 12, 5462)
