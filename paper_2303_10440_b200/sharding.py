@@ -37,8 +37,10 @@ def sharded_mesh_ft_backward(plan, vertices, dL_dF, group=None):
     begin, end = slab_bounds(plan.n[0], world, rank)
     if end > begin:
         plan.set_slab(begin, end)
-        dv = plan.mesh_ft_backward(vertices, dL_dF)
-        plan.set_slab(0, plan.n[0])
+        try:
+            dv = plan.mesh_ft_backward(vertices, dL_dF)
+        finally:   # a failed call must not leave the plan on a partial slab (every later render would be refused)
+            plan.set_slab(0, plan.n[0])
     else:  # more ranks than rows: nothing to reduce here
         import torch
 
@@ -46,11 +48,14 @@ def sharded_mesh_ft_backward(plan, vertices, dL_dF, group=None):
     return allreduce_vertex_gradient(dv, group)
 
 
-def allgather_spectrum_slabs(F, group=None):
+def allgather_spectrum_slabs(F, group=None, buffers=None):
     """All-gather of the x-slabs of a spectrum tensor F [n_x, n_y, n_z/2+1] (complex or real, CPU or CUDA), in place:
     on entry every rank holds valid rows ``slab_bounds(n_x, world, rank)`` of F, on return every rank holds all rows.
     Needed only when a rank goes on to the inverse FFT.  Slabs differ by at most one row, so they
-    are padded to the largest and exchanged with ONE all_gather_into_tensor (<= 68 MB at config 5)."""
+    are padded to the largest and exchanged with ONE all_gather_into_tensor (<= 68 MB at config 5).
+    ``buffers``: a dict the caller keeps between calls; the padded send buffer and the receive buffer (together about twice
+    the spectrum) are created in it on first use and reused afterwards, instead of being allocated on every call (inside a
+    timed step, at config 5, that is 2 x 68 MB per call).  ``None`` allocates fresh buffers."""
     import torch
     import torch.distributed as dist
 
@@ -60,10 +65,16 @@ def allgather_spectrum_slabs(F, group=None):
     n_x = F.shape[0]
     rows = max(slab_bounds(n_x, world, r)[1] - slab_bounds(n_x, world, r)[0] for r in range(world))
     Fr = torch.view_as_real(F) if F.is_complex() else F
-    send = torch.zeros((rows,) + tuple(Fr.shape[1:]), dtype=Fr.dtype, device=Fr.device)
+    key = (tuple(Fr.shape), Fr.dtype, Fr.device, world)
+    if buffers is not None and key in buffers:
+        send, recv = buffers[key]
+    else:
+        send = torch.zeros((rows,) + tuple(Fr.shape[1:]), dtype=Fr.dtype, device=Fr.device)   # padding rows stay zero
+        recv = torch.empty((world * rows,) + tuple(Fr.shape[1:]), dtype=Fr.dtype, device=Fr.device)
+        if buffers is not None:
+            buffers[key] = (send, recv)
     b, e = slab_bounds(n_x, world, rank)
     send[: e - b] = Fr[b:e]
-    recv = torch.empty((world * rows,) + tuple(Fr.shape[1:]), dtype=Fr.dtype, device=Fr.device)
     dist.all_gather_into_tensor(recv, send, group=group)
     for r in range(world):
         rb, re_ = slab_bounds(n_x, world, r)
@@ -86,6 +97,21 @@ def sharded_mesh_ft_forward(plan, vertices, out=None, group=None, gather=True):
         out = torch.zeros(plan.spectrum_shape, dtype=torch.complex64, device=plan.device)
     if end > begin:
         plan.set_slab(begin, end)
-        plan.mesh_ft_forward(vertices, out=out)
-        plan.set_slab(0, plan.n[0])
-    return allgather_spectrum_slabs(out, group) if gather else out
+        try:
+            plan.mesh_ft_forward(vertices, out=out)
+        finally:   # a failed call must not leave the plan on a partial slab (every later render would be refused)
+            plan.set_slab(0, plan.n[0])
+    return allgather_spectrum_slabs(out, group, buffers=_plan_gather_buffers(plan)) if gather else out
+
+
+def _plan_gather_buffers(plan):
+    """The dict in which allgather_spectrum_slabs keeps its send / receive buffers for this plan (one pair per spectrum
+    shape, dtype, device and world size), so that a loop of sharded forwards allocates them once, not every step."""
+    cache = getattr(plan, "_gather_buffers", None)
+    if cache is None:
+        cache = {}
+        try:
+            plan._gather_buffers = cache
+        except AttributeError:   # a plan type without instance attributes: no caching
+            return None
+    return cache

@@ -116,6 +116,31 @@ def _worker(rank, world, port, out_dir):
             Fs2 = sharded_mesh_ft_forward(plan, vt, out=torch.zeros(w.spectrum_shape, dtype=torch.complex64))
             dv2 = sharded_mesh_ft_backward(plan, vt, torch.as_tensor(G.astype(np.complex64)))
             assert plan.slab == (0, nx)                                     # the plan is handed back on the whole grid
+            # a second sharded forward reuses the gather buffers kept on the plan (no per-step allocation), same result
+            bufs = {k: (s_.data_ptr(), r_.data_ptr()) for k, (s_, r_) in plan._gather_buffers.items()}
+            assert len(bufs) == 1
+            Fs3 = sharded_mesh_ft_forward(plan, vt, out=torch.full(w.spectrum_shape, float("nan"), dtype=torch.complex64))
+            assert {k: (s_.data_ptr(), r_.data_ptr()) for k, (s_, r_) in plan._gather_buffers.items()} == bufs
+            assert torch.equal(Fs3, Fs2)
+            # a call that raises still hands the plan back on the whole grid (no collective is pending: it fails before it)
+            class _Boom(RuntimeError):
+                pass
+
+            def _raise(*a, **k):
+                raise _Boom()
+
+            if e > b:
+                good_fwd, good_bwd = plan.mesh_ft_forward, plan.mesh_ft_backward
+                plan.mesh_ft_forward = plan.mesh_ft_backward = _raise
+                for call in (lambda: sharded_mesh_ft_forward(plan, vt, out=torch.zeros(w.spectrum_shape, dtype=torch.complex64), gather=False),
+                             lambda: sharded_mesh_ft_backward(plan, vt, torch.as_tensor(G.astype(np.complex64)))):
+                    try:
+                        call()
+                        raise AssertionError("the stand-in kernel call should have raised")
+                    except _Boom:
+                        pass
+                    assert plan.slab == (0, nx)
+                plan.mesh_ft_forward, plan.mesh_ft_backward = good_fwd, good_bwd
             np.save(os.path.join(out_dir, f"Fs2_{mode}_{rank}.npy"), Fs2.numpy())
             np.save(os.path.join(out_dir, f"dv2_{mode}_{rank}.npy"), dv2.numpy())
             np.save(os.path.join(out_dir, f"dv_{mode}_{rank}.npy"), dv.numpy())
