@@ -209,8 +209,10 @@ void dm_plan_destroy(dm_plan* plan);
  *   g~    = (I + lambda L)^-2 g                         L = D - A, the connectivity Laplacian of the mesh's vertex graph;
  *                                                       two conjugate-gradient solves with I + lambda L on the device
  *                                                       (the paper uses a sparse Cholesky factorisation), fp64; one
- *                                                       persistent cooperative kernel per solve when the mesh fits one
- *                                                       resident grid (~3e5 vertices), else three launches per iteration
+ *                                                       persistent cooperative kernel per solve wherever the device
+ *                                                       supports cooperative launches (its blocks stride over the vertex
+ *                                                       tiles when the mesh has more tiles than one resident grid,
+ *                                                       ~3e5 vertices), else three launches per iteration
  *   vertices <- AdamUniform(vertices, g~)               m_t = b1 m + (1-b1) g~,  s_t = b2 s + (1-b2) max_i g~_i^2,
  *                                                       v -= lr (m_t/(1-b1^t)) / (sqrt(s_t/(1-b2^t)) + eps)
  * The state owns the vertex graph, the optimiser moments (zero at creation) and all scratch; it belongs to ONE plan
@@ -228,9 +230,11 @@ typedef struct dm_shape_params {
     float   cg_tol;      /* a solve stops when |r| <= cg_tol |b| on every column (default 1e-7)       */
     int32_t cg_max_iter; /* at most this many iterations are queued per solve (default 400); fewer when
                             the convergence bound of CG for cond(I + lambda L) <= 1 + 2 lambda d_max says so */
-    int32_t solver;      /* 0 = automatic (default): one persistent cooperative kernel per solve when the whole solve
-                            fits one resident grid, else 1;  1 = three launches per iteration (same arithmetic, same
-                            results bit for bit while every vertex tile has its own block) */
+    int32_t solver;      /* 0 = automatic (default): one persistent cooperative kernel per solve whenever the device
+                            supports cooperative launches (a refused launch falls back to 1);  1 = three launches per
+                            iteration.  Same arithmetic; the results agree bit for bit while every 256-vertex tile has a
+                            block of its own in the resident grid (~3e5 vertices on a B200) -- beyond that the persistent
+                            solve sums its dot products in a different order and the two differ by rounding */
 } dm_shape_params;
 
 int dm_shape_params_default(dm_shape_params* out);
@@ -242,9 +246,16 @@ int dm_shape_state_create(dm_plan* plan, const dm_shape_params* params, dm_shape
 int dm_shape_precondition(dm_plan* plan, dm_shape_state* state, const float* g_dev, float* out_dev);
 
 /* Conjugate-gradient iterations the two solves of the last dm_shape_precondition / dm_shape_step took (iters[0], iters[1]);
- * -1 when the solves ran as separate launches (meshes too large for one resident grid), which keep no count.
+ * -1 when the solves ran as separate launches (solver = 1, or a refused cooperative launch), which keep no count.
  * Synchronises the stream. */
 int dm_shape_last_cg_iterations(dm_plan* plan, dm_shape_state* state, int32_t iters[2]);
+
+/* How well those two solves converged: rel[i] = max over the three columns of |r| / |b| when solve i stopped (0 before
+ * any solve).  Both solver forms stop silently after cg_max_iter iterations (a large lambda needs more: the iteration
+ * count grows like sqrt(1 + 2 lambda d_max)); *converged (may be NULL) is 1 when both rel[i] <= cg_tol, 0 when a solve
+ * ran out of iterations first -- the step was then taken with an inexactly preconditioned gradient.  Synchronises the
+ * stream. */
+int dm_shape_last_cg_residuals(dm_plan* plan, dm_shape_state* state, double rel[2], int32_t* converged);
 
 /* One step.  vertices_dev float32 [n_vertices*3] is updated IN PLACE; target_dev float32 [n_x*n_y*n_z] is the image m;
  * psf_cov_host as in dm_render.  loss_host = NULL, or a HOST double that receives Phi_1 of the vertices BEFORE the

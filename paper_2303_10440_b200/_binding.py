@@ -16,7 +16,7 @@ _SYMBOLS = (
     "dm_plan_create", "dm_plan_set_stream", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_mesh_ft_backward_with_spectrum", "dm_render",
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
     "dm_plan_launch_count", "dm_plan_paths_used", "dm_plan_destroy", "dm_error_string", "dm_version",
-    "dm_shape_params_default", "dm_shape_state_create", "dm_shape_precondition", "dm_shape_last_cg_iterations", "dm_shape_step", "dm_shape_state_destroy",
+    "dm_shape_params_default", "dm_shape_state_create", "dm_shape_precondition", "dm_shape_last_cg_iterations", "dm_shape_last_cg_residuals", "dm_shape_step", "dm_shape_state_destroy",
     "dm_mesh_ft_forward_noalloc",
 )
 DM_NOALLOC_MAX_FACES = 65536
@@ -88,6 +88,7 @@ def load_library():
     lib.dm_shape_state_create.argtypes = [vp, ctypes.POINTER(ShapeParams), ctypes.POINTER(vp)]
     lib.dm_shape_precondition.argtypes = [vp, vp, fp, fp]
     lib.dm_shape_last_cg_iterations.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_int32)]
+    lib.dm_shape_last_cg_residuals.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)]
     lib.dm_shape_step.argtypes = [vp, vp, fp, fp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_double)]
     lib.dm_shape_state_destroy.argtypes = [vp]
     lib.dm_shape_state_destroy.restype = None
@@ -172,6 +173,9 @@ class Plan:
         self.n_faces = int(faces.shape[0])
         self.device = faces.device
         self.stream = torch.cuda.current_stream(self.device) if stream is None else stream
+        # bookkeeping for the autograd front end (state_epoch): how often the plan's configuration changed, how many forward
+        # spectra it has produced, and whether backward calls take the spectrum of the last render (DM_OPT_REUSE_SPECTRUM)
+        self._config_epoch, self._forward_epoch, self._reuse_spectrum = 0, 0, False
         g = _Grid()
         for d in range(3):
             g.n[d] = self.n[d]
@@ -211,20 +215,33 @@ class Plan:
         self.stream = self._torch.cuda.current_stream(self.device) if stream is None else stream
         _check(self._lib.dm_plan_set_stream(self._h, self.stream.cuda_stream), "dm_plan_set_stream")
 
+    def state_epoch(self):
+        """A token that changes whenever a later backward call on this plan would differentiate a different function than
+        a forward call made now: after set_slab / set_face_weights / set_narrow_band / set_option, and -- only under
+        DM_OPT_REUSE_SPECTRUM, where the backward takes F from the last render -- after any other forward, render or shape
+        step.  autograd.py compares the token of its forward with the one at backward time."""
+        return (self._config_epoch, self._forward_epoch if self._reuse_spectrum else None)
+
     def set_slab(self, ix_begin: int, ix_end: int):
+        self._config_epoch += 1
         _check(self._lib.dm_plan_set_slab(self._h, int(ix_begin), int(ix_end)), "dm_plan_set_slab")
 
     def set_face_weights(self, weights=None):
         """Per-face density weights (float32 CUDA tensor [n_faces]); ``None`` = all 1."""
         ptr = None if weights is None else self._f32(weights, self.n_faces, "face weights").data_ptr()
+        self._config_epoch += 1
         _check(self._lib.dm_plan_set_face_weights(self._h, ptr), "dm_plan_set_face_weights")
 
     def set_narrow_band(self, psf_cov=None, cutoff: float = 0.01):
         """Evaluate only the frequencies with exp(-1/2 k^T B k) > cutoff; ``psf_cov=None`` = off."""
+        self._config_epoch += 1
         _check(self._lib.dm_plan_set_narrow_band(self._h, None if psf_cov is None else _cov(psf_cov), float(cutoff)),
                "dm_plan_set_narrow_band")
 
     def set_option(self, option: int, value: float):
+        self._config_epoch += 1
+        if int(option) == DM_OPT_REUSE_SPECTRUM:
+            self._reuse_spectrum = bool(value)
         _check(self._lib.dm_plan_set_option(self._h, int(option), float(value)), "dm_plan_set_option")
 
     def mesh_ft_forward(self, vertices, out=None):
@@ -233,6 +250,7 @@ class Plan:
         if out is None:
             out = torch.zeros(self.spectrum_shape, dtype=torch.complex64, device=self.device)
         o = self._f32(out, 2 * self._nk(), "F")
+        self._forward_epoch += 1
         _check(self._lib.dm_mesh_ft_forward(self._h, v.data_ptr(), o.data_ptr()), "dm_mesh_ft_forward")
         return out
 
@@ -258,6 +276,7 @@ class Plan:
         if out is None:
             out = torch.empty(self.n, dtype=torch.float32, device=self.device)
         o = self._f32(out, self.n[0] * self.n[1] * self.n[2], "image")
+        self._forward_epoch += 1
         _check(self._lib.dm_render(self._h, v.data_ptr(), _cov(psf_cov), o.data_ptr()), "dm_render")
         return out
 
@@ -359,12 +378,21 @@ class ShapeState:
         _check(self._lib.dm_shape_last_cg_iterations(self._plan._h, self._h, out), "dm_shape_last_cg_iterations")
         return int(out[0]), int(out[1])
 
+    def last_cg_residuals(self):
+        """((rel0, rel1), converged): max-over-columns |r|/|b| the two solves of the last precondition / step stopped at, and
+        whether both met cg_tol (False: a solve ran out of cg_max_iter iterations).  Synchronises."""
+        rel = (ctypes.c_double * 2)()
+        ok = ctypes.c_int32(0)
+        _check(self._lib.dm_shape_last_cg_residuals(self._plan._h, self._h, rel, ctypes.byref(ok)), "dm_shape_last_cg_residuals")
+        return (float(rel[0]), float(rel[1])), bool(ok.value)
+
     def step(self, vertices, target, psf_cov, return_loss: bool = False):
         """One step; ``vertices`` is updated in place.  With ``return_loss`` returns Phi_1 before the step (synchronises)."""
         p = self._plan
         v = p._vertices(vertices)
         t = p._f32(target, p.n[0] * p.n[1] * p.n[2], "target")
         loss = ctypes.c_double() if return_loss else None
+        p._forward_epoch += 1
         _check(self._lib.dm_shape_step(p._h, self._h, v.data_ptr(), t.data_ptr(), _cov(psf_cov),
                                        ctypes.byref(loss) if return_loss else None), "dm_shape_step")
         return float(loss.value) if return_loss else None

@@ -961,6 +961,7 @@ struct dm_shape_state {
     int cg_iter_bound = 0;           // iterations after which CG has converged to cg_tol whatever the right-hand side
     int coop_blocks = 0;             // > 0: blocks of the persistent (cooperative) solve; 0: the multi-launch solve
     int* cg_iters = nullptr;         // [2] device: iterations the two solves of the last preconditioning took (persistent solve)
+    double* cg_res = nullptr;        // [2] device: relative residual max_c |r|/|b| the two solves ended with (both solve forms)
     double *mom = nullptr, *amax_part = nullptr, *s_next = nullptr;
     DmAdamScalars* adam = nullptr;
     float *image = nullptr, *cot = nullptr, *grad = nullptr;
@@ -979,9 +980,10 @@ int shape_cg_solve(dm_plan* p, dm_shape_state* st, const TB* b_dev, double* x_de
         int n_ = n, max_iter = st->prm.cg_max_iter;
         double lambda = (double)st->prm.lambda, tol2_ = (double)st->prm.cg_tol * (double)st->prm.cg_tol;
         int* iters = st->cg_iters + which;
+        double* res = st->cg_res + which;
         void* args[] = {(void*)&st->adj_off, (void*)&st->adj_idx, (void*)&n_, (void*)&lambda, (void*)&b_dev, (void*)&x_dev,
                         (void*)&st->cg_r, (void*)&st->cg_p, (void*)&st->cg_Ap, (void*)&st->part_a, (void*)&st->part_b,
-                        (void*)&tol2_, (void*)&max_iter, (void*)&iters};
+                        (void*)&tol2_, (void*)&max_iter, (void*)&iters, (void*)&res};
         if (cudaLaunchCooperativeKernel((const void*)dm_k_cg_persistent<TB>, dim3((unsigned)st->coop_blocks), dim3(DM_SH_THREADS),
                                         args, 0, p->stream) == cudaSuccess)
             return check_launch(p, 1);
@@ -1004,7 +1006,9 @@ int shape_cg_solve(dm_plan* p, dm_shape_state* st, const TB* b_dev, double* x_de
         dm_k_cg_update_p<<<nb, DM_SH_THREADS, 0, p->stream>>>(n, st->cg_r, st->cg_p, st->part_b, nb, sc, sc_next, tol2);
         rc = check_launch(p, 3);
     }
-    return rc;
+    if (rc) return rc;
+    dm_k_cg_residual<<<1, 1, 0, p->stream>>>(st->cg_sc + (n_iter & 1), st->cg_res + which);
+    return check_launch(p);
 }
 
 // out = (I + lambda L)^-2 g: two solves (reading R27); the result stays in st->cg_x (fp64)
@@ -1092,7 +1096,7 @@ int dm_shape_state_create(dm_plan* p, const dm_shape_params* params, dm_shape_st
             cudaMalloc(&st->cg_r, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->cg_p, n3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->cg_Ap, n3 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->part_a, nb3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->part_b, nb3 * sizeof(double)) != cudaSuccess ||
-            cudaMalloc(&st->cg_sc, 2 * sizeof(DmCgScalars)) != cudaSuccess || cudaMalloc(&st->cg_iters, 2 * sizeof(int)) != cudaSuccess || cudaMalloc(&st->mom, n3 * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&st->cg_sc, 2 * sizeof(DmCgScalars)) != cudaSuccess || cudaMalloc(&st->cg_iters, 2 * sizeof(int)) != cudaSuccess || cudaMalloc(&st->cg_res, 2 * sizeof(double)) != cudaSuccess || cudaMalloc(&st->mom, n3 * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->amax_part, DM_SH_LOSS_BLOCKS * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&st->s_next, sizeof(double)) != cudaSuccess || cudaMalloc(&st->adam, sizeof(DmAdamScalars)) != cudaSuccess ||
             cudaMalloc(&st->image, nvox * sizeof(float)) != cudaSuccess || cudaMalloc(&st->cot, nvox * sizeof(float)) != cudaSuccess ||
@@ -1105,6 +1109,7 @@ int dm_shape_state_create(dm_plan* p, const dm_shape_params* params, dm_shape_st
             cudaMemsetAsync(st->mom, 0, n3 * sizeof(double), p->stream) != cudaSuccess ||
             cudaMemsetAsync(st->adam, 0, sizeof(DmAdamScalars), p->stream) != cudaSuccess ||
             cudaMemsetAsync(st->cg_iters, 0, 2 * sizeof(int), p->stream) != cudaSuccess ||
+            cudaMemsetAsync(st->cg_res, 0, 2 * sizeof(double), p->stream) != cudaSuccess ||
             cudaStreamSynchronize(p->stream) != cudaSuccess) { rc = DM_ERR_CUDA; break; }
         // the persistent solve needs every block resident at once (cooperative launch); blocks stride over the vertex tiles
         {
@@ -1151,6 +1156,16 @@ int dm_shape_last_cg_iterations(dm_plan* p, dm_shape_state* st, int32_t iters[2]
         return DM_ERR_CUDA;
     iters[0] = h[0];
     iters[1] = h[1];
+    return DM_OK;
+}
+
+int dm_shape_last_cg_residuals(dm_plan* p, dm_shape_state* st, double rel[2], int32_t* converged)
+{
+    if (!p || !st || st->plan != p || !rel) return DM_ERR_INVALID_ARG;
+    if (cudaMemcpyAsync(rel, st->cg_res, 2 * sizeof(double), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess ||
+        cudaStreamSynchronize(p->stream) != cudaSuccess)
+        return DM_ERR_CUDA;
+    if (converged) *converged = (rel[0] <= (double)st->prm.cg_tol && rel[1] <= (double)st->prm.cg_tol) ? 1 : 0;
     return DM_OK;
 }
 
@@ -1201,6 +1216,7 @@ void dm_shape_state_destroy(dm_shape_state* st)
     cudaFree(st->part_b);
     cudaFree(st->cg_sc);
     cudaFree(st->cg_iters);
+    cudaFree(st->cg_res);
     cudaFree(st->mom);
     cudaFree(st->amax_part);
     cudaFree(st->s_next);

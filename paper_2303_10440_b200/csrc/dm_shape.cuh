@@ -86,6 +86,15 @@ struct DmCgScalars {
     int done;       // every column has r.r <= tol^2 b.b
 };
 
+// max over the three columns of |r| / |b| (0 for a zero right-hand side)
+__device__ __forceinline__ double dm_sh_rel_residual(const double rr[3], const double bb[3])
+{
+    double m = 0.0;
+    for (int c = 0; c < 3; ++c)
+        if (bb[c] > 0.0) m = fmax(m, sqrt(rr[c] / bb[c]));
+    return m;
+}
+
 // x = 0, r = p = b (b given as fp32 [n][3] or fp64), partial r.r
 template <typename TB>
 __global__ void __launch_bounds__(DM_SH_THREADS)
@@ -299,7 +308,7 @@ __global__ void __launch_bounds__(DM_SH_THREADS)
 dm_k_cg_persistent(const int32_t* __restrict__ adj_off, const int32_t* __restrict__ adj_idx, int n, double lambda,
                    const TB* __restrict__ b, double* __restrict__ x, double* __restrict__ r, double* __restrict__ p,
                    double* __restrict__ Ap, double* __restrict__ part_a, double* __restrict__ part_b, double tol2, int max_iter,
-                   int* __restrict__ iters_out)
+                   int* __restrict__ iters_out, double* __restrict__ res_out)
 {
     __shared__ double sh[3][DM_SH_THREADS];
     const int stride = (int)gridDim.x * DM_SH_THREADS;
@@ -355,5 +364,14 @@ dm_k_cg_persistent(const int32_t* __restrict__ adj_off, const int32_t* __restric
         for (int c = 0; c < 3; ++c) rr[c] = rn[c];
         cooperative_groups::this_grid().sync();   // p is complete before the next product reads the neighbours
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0 && iters_out) *iters_out = it;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        if (iters_out) *iters_out = it;
+        if (res_out) *res_out = dm_sh_rel_residual(rr, bb);
+    }
+}
+
+// the relative residual the multi-launch solve ended with (its scalars live in sc)
+__global__ void dm_k_cg_residual(const DmCgScalars* __restrict__ sc, double* __restrict__ res_out)
+{
+    *res_out = dm_sh_rel_residual(sc->rr, sc->bb);
 }

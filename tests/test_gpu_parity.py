@@ -654,4 +654,18 @@ def test_autograd_front_end(dm):
     img = dm.render(plan, v, w.psf_cov)
     (gv2,) = torch.autograd.grad(((img - target) ** 2).sum(), v)
     assert torch.equal(gv2, dv)
+    # a plan that changed between forward and backward is refused (the gradient would be the banded function's)
+    img = dm.render(plan, v, w.psf_cov)
+    plan.set_narrow_band(w.psf_cov, 0.01)
+    with pytest.raises(RuntimeError, match="plan changed between forward and backward"):
+        torch.autograd.grad(((img - target) ** 2).sum(), v)
+    plan.set_narrow_band(None)
+    # with DM_OPT_REUSE_SPECTRUM the backward reads the spectrum of the LAST render: one in between invalidates the graph
+    plan.set_option(dm.DM_OPT_REUSE_SPECTRUM, 1)
+    img = dm.render(plan, v, cov)
+    (gv3, gc3) = torch.autograd.grad(((img - target) ** 2).sum(), (v, cov), retain_graph=True)
+    assert torch.allclose(gv3, dv, rtol=1e-5, atol=1e-6 * float(dv.abs().max())) and np.allclose(gc3.numpy(), np.array(dcov, dtype=np.float32), rtol=1e-5)
+    plan.render(_dev(w.vertices * 0.9), w.psf_cov)
+    with pytest.raises(RuntimeError, match="plan changed between forward and backward"):
+        torch.autograd.grad(((img - target) ** 2).sum(), (v, cov))
     plan.close()

@@ -48,6 +48,18 @@ def test_preconditioner_against_dense_solves(dm, cfg, sub):
         out3 = st2.precondition(torch.as_tensor(g, device="cuda")).cpu().numpy()
         assert st2.last_cg_iterations() == (-1, -1)
         assert np.array_equal(out, out3)
+        # both forms report the residual they stopped at, and that they converged
+        for s_ in (st, st2):
+            rel, ok = s_.last_cg_residuals()
+            assert ok and all(0.0 <= r <= 1e-7 for r in rel), rel
+        assert st.last_cg_residuals() == st2.last_cg_residuals()
+        if lam == 50.0:
+            # a solve cut short is reported, not hidden: two iterations cannot reach 1e-7 at lambda = 50
+            st3 = plan.shape_state(lambda_=lam, cg_max_iter=2)
+            st3.precondition(torch.as_tensor(g, device="cuda"))
+            rel3, ok3 = st3.last_cg_residuals()
+            assert not ok3 and max(rel3) > 1e-7 and st3.last_cg_iterations() == (2, 2)
+            st3.close()
         st2.close()
         st.close()
     plan.close()
