@@ -100,6 +100,17 @@ int dm_plan_set_slab(dm_plan* plan, int32_t ix_begin, int32_t ix_end);
  * return DM_ERR_INVALID_ARG. */
 int dm_plan_set_face_weights(dm_plan* plan, const float* weights_dev);
 
+/* The same for a loop that refits the densities every step and cannot afford a stream
+ * synchronisation and a host pass over the weights per step: copies weights_dev (device float32 [n_faces], not NULL)
+ * asynchronously on the plan's stream and reads nothing back.  The caller states the class instead of having it
+ * detected:  robust = 0 promises what dm_plan_set_face_weights checks for the fast kernels -- all weights finite and of
+ * one sign and, in DM_VOLUME, equal on all faces of a connected component -- and robust = 1 sends every pair through
+ * the robust kernels (always valid, several times slower).  A broken promise is not detected; the result may then miss
+ * the tolerance.  Typical use: one dm_plan_set_face_weights call up front (allocates the plan's copy, classifies; read the
+ * class back with dm_plan_paths_used after a forward), then this call inside the loop; once the plan's copy exists the
+ * call allocates nothing and nothing in it synchronises. */
+int dm_plan_update_face_weights(dm_plan* plan, const float* weights_dev, int32_t robust);
+
 /* Narrow band ("evaluate the FT only where the PSF spectrum is above 1 % of its maximum").
  * With psf_cov_host = 6 floats on the HOST (covariance B of a Gaussian PSF, order xx, yy, zz, xy, xz, yz) and
  * 0 < cutoff < 1, the mesh-FT calls of this plan evaluate only the stored frequencies with

@@ -13,7 +13,7 @@ DM_OPT_REUSE_SPECTRUM = 5
 
 # every symbol include/deltamic.h declares
 _SYMBOLS = (
-    "dm_plan_create", "dm_plan_set_stream", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_mesh_ft_backward_with_spectrum", "dm_render",
+    "dm_plan_create", "dm_plan_set_stream", "dm_plan_set_slab", "dm_plan_set_narrow_band", "dm_plan_set_face_weights", "dm_plan_update_face_weights", "dm_plan_set_option", "dm_mesh_ft_forward", "dm_mesh_ft_backward", "dm_mesh_ft_backward_with_spectrum", "dm_render",
     "dm_render_backward", "dm_spectrum_to_image", "dm_image_to_spectrum_cotangent", "dm_plan_stage_ms",
     "dm_plan_launch_count", "dm_plan_paths_used", "dm_plan_destroy", "dm_error_string", "dm_version",
     "dm_shape_params_default", "dm_shape_state_create", "dm_shape_precondition", "dm_shape_last_cg_iterations", "dm_shape_last_cg_residuals", "dm_shape_step", "dm_shape_state_destroy",
@@ -67,6 +67,7 @@ def load_library():
     lib.dm_plan_set_slab.argtypes = [vp, ctypes.c_int32, ctypes.c_int32]
     lib.dm_plan_set_option.argtypes = [vp, ctypes.c_int, ctypes.c_double]
     lib.dm_plan_set_face_weights.argtypes = [vp, fp]
+    lib.dm_plan_update_face_weights.argtypes = [vp, fp, ctypes.c_int32]
     lib.dm_plan_set_narrow_band.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.c_float]
     lib.dm_mesh_ft_forward.argtypes = [vp, fp, fp]
     lib.dm_mesh_ft_backward.argtypes = [vp, fp, fp, fp]
@@ -231,6 +232,13 @@ class Plan:
         ptr = None if weights is None else self._f32(weights, self.n_faces, "face weights").data_ptr()
         self._config_epoch += 1
         _check(self._lib.dm_plan_set_face_weights(self._h, ptr), "dm_plan_set_face_weights")
+
+    def update_face_weights(self, weights, robust: bool = False):
+        """dm_plan_update_face_weights: new weights without the classification pass and its stream synchronisation; the
+        caller asserts their class (``robust=False``: one sign, constant per component in volume mode)."""
+        ptr = self._f32(weights, self.n_faces, "face weights").data_ptr()
+        self._config_epoch += 1
+        _check(self._lib.dm_plan_update_face_weights(self._h, ptr, 1 if robust else 0), "dm_plan_update_face_weights")
 
     def set_narrow_band(self, psf_cov=None, cutoff: float = 0.01):
         """Evaluate only the frequencies with exp(-1/2 k^T B k) > cutoff; ``psf_cov=None`` = off."""

@@ -645,6 +645,19 @@ int dm_plan_set_face_weights(dm_plan* p, const float* weights_dev)
     return DM_OK;
 }
 
+int dm_plan_update_face_weights(dm_plan* p, const float* weights_dev, int32_t robust)
+{
+    if (!p || !weights_dev || (robust != 0 && robust != 1)) return DM_ERR_INVALID_ARG;
+    p->F_valid = false;
+    if (!p->face_w && cudaMalloc(&p->face_w, (size_t)p->n_faces * sizeof(float)) != cudaSuccess) return DM_ERR_ALLOC;
+    if (cudaMemcpyAsync(p->face_w, weights_dev, (size_t)p->n_faces * sizeof(float), cudaMemcpyDeviceToDevice, p->stream) !=
+        cudaSuccess)
+        return DM_ERR_CUDA;
+    p->gd.face_w = p->face_w;
+    p->weights_robust = robust != 0;   // the caller's word: nothing is read back
+    return DM_OK;
+}
+
 int dm_plan_set_narrow_band(dm_plan* p, const float* psf_cov_host, float cutoff)
 {
     if (!p) return DM_ERR_INVALID_ARG;

@@ -86,7 +86,7 @@ def test_plan_state_epoch_moves_with_every_setter():
     """The real Plan's bookkeeping, without a device: the setters bump the epoch before they reach the library."""
     import paper_2303_10440_b200._binding as b
     src = open(b.__file__).read()
-    for name in ("set_slab", "set_face_weights", "set_narrow_band", "set_option"):
+    for name in ("set_slab", "set_face_weights", "update_face_weights", "set_narrow_band", "set_option"):
         body = src[src.index(f"    def {name}("):]
         body = body[:body.index("\n    def ", 1)]
         assert "self._config_epoch += 1" in body, name

@@ -41,7 +41,7 @@ def _rel_l2(a, b):
 
 
 @pytest.mark.parametrize("cfg", [2, 3, 4, 5])
-def test_forward_sampled_frequencies(dm, cfg):
+def test_forward_sampled_frequencies(dm, cfg, report):
     w, plan, vd = _setup(dm, cfg)
     F = plan.mesh_ft_forward(vd).cpu().numpy()
     assert np.isfinite(F.view(np.float32)).all()
@@ -49,7 +49,7 @@ def test_forward_sampled_frequencies(dm, cfg):
     ref = oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, w.mode, flat_indices=idx)
     f0 = abs(oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, w.mode, flat_indices=np.array([0]))[0])
     err = np.abs(F.reshape(-1)[idx] - ref).max() / f0
-    print(f"cfg{cfg} forward: max|dF|/|F(0)| = {err:.2e} over {len(idx)} sampled frequencies")
+    report(f"cfg{cfg} forward: max|dF|/|F(0)| = {err:.2e} over {len(idx)} sampled frequencies")
     assert err <= FWD_TOL, err
     # F(-kx,-ky,0) = conj F(kx,ky,0) inside the stored grid (any size; pin P3)
     nx, ny = w.n[0], w.n[1]
@@ -63,7 +63,7 @@ def test_forward_sampled_frequencies(dm, cfg):
 
 
 @pytest.mark.parametrize("cfg", [2, 3, 4, 5])
-def test_backward_sampled_frequencies(dm, cfg):
+def test_backward_sampled_frequencies(dm, cfg, report):
     import torch
     w, plan, vd = _setup(dm, cfg)
     idx = sampled_frequencies(w, n_random=768 if cfg < 5 else 384, n_nyquist=32)
@@ -77,15 +77,16 @@ def test_backward_sampled_frequencies(dm, cfg):
     ref = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, w.mode, Gs.astype(np.complex128),
                                        flat_indices=idx)
     err = _rel_l2(dv, ref)
-    print(f"cfg{cfg} backward: rel L2 = {err:.2e} over {len(idx)} sampled frequencies")
+    report(f"cfg{cfg} backward: rel L2 = {err:.2e} over {len(idx)} sampled frequencies")
     assert err <= GRAD_TOL, err
     plan.close()
 
 
-@pytest.mark.parametrize("cfg", [3, 4])
-def test_fast_kernels_match_robust_kernels_whole_grid(dm, cfg):
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_fast_kernels_match_robust_kernels_whole_grid(dm, cfg, report):
     """Every (triangle, frequency) pair of the full config: the fast kernels against the kernels that send every pair
-    through the series / far-pair branches (which the tests of test_gpu_parity.py tie to the oracle)."""
+    through the series / far-pair branches (which the tests of test_gpu_parity.py tie to the oracle).  Config 5 is the only
+    one on the SEG = 16 instantiation of the fast backward kernel (72 < n_z/2+1 = 129 <= 144)."""
     import torch
     from workloads.configs import spectrum_cotangent
     w, plan, vd = _setup(dm, cfg)
@@ -101,9 +102,41 @@ def test_fast_kernels_match_robust_kernels_whole_grid(dm, cfg):
     f0 = float(Fr[0, 0, 0].abs())
     ferr = float((F - Fr).abs().max()) / f0
     gerr = float(torch.linalg.norm(dv - dvr) / torch.linalg.norm(dvr))
-    print(f"cfg{cfg} fast vs robust over the whole grid: forward {ferr:.2e} |F(0)|, gradient rel L2 {gerr:.2e}")
+    report(f"cfg{cfg} fast vs robust over the whole grid: forward {ferr:.2e} |F(0)|, gradient rel L2 {gerr:.2e}")
     assert ferr <= 0.5 * FWD_TOL
     assert gerr <= 0.5 * GRAD_TOL
+    plan.close()
+
+
+def test_cfg3_complete_x_rows_against_the_oracle(dm, report):
+    """Config 3 (40 960 triangles, 128 x 128 x 64) against the oracle on EVERY stored frequency of complete x-rows -- rows 0..15
+    (the low frequencies, where the series branches live), the Nyquist row and the last row (n_x = -1): 18 x 4224 frequencies,
+    about a minute of oracle time -- instead of a sample; and the backward with a cotangent that lives on three complete rows
+    (the oracle's backward costs about five times its forward per frequency)."""
+    import torch
+    w, plan, vd = _setup(dm, 3)
+    nx, ny, nzh = w.spectrum_shape
+    F = plan.mesh_ft_forward(vd).cpu().numpy()
+    rows = list(range(16)) + [nx // 2, nx - 1]
+    per_row = ny * nzh
+    idx = np.concatenate([np.arange(r * per_row, (r + 1) * per_row, dtype=np.int64) for r in rows])
+    ref = oracle.mesh_ft_forward_grid(w.vertices, w.faces, w.n, w.spacing, w.mode, flat_indices=idx)
+    f0 = abs(ref[0])
+    err_rows = np.abs(F.reshape(-1)[idx] - ref).reshape(len(rows), per_row).max(axis=1) / f0
+    report(f"cfg3 forward, complete x-rows {rows[0]}..{rows[15]}, {rows[16]}, {rows[17]} ({len(idx)} frequencies): "
+           f"max|dF|/|F(0)| = {err_rows.max():.2e} (worst row {rows[int(err_rows.argmax())]})")
+    assert err_rows.max() <= FWD_TOL, err_rows
+    brows = [0, 1, nx // 2]
+    bidx = np.concatenate([np.arange(r * per_row, (r + 1) * per_row, dtype=np.int64) for r in brows])
+    rng = np.random.default_rng(3003)
+    Gs = (rng.standard_normal(len(bidx)) + 1j * rng.standard_normal(len(bidx))).astype(np.complex64)
+    G = np.zeros(w.n_k, dtype=np.complex64)
+    G[bidx] = Gs
+    dv = plan.mesh_ft_backward(vd, torch.as_tensor(G.reshape(w.spectrum_shape), device="cuda")).cpu().numpy()
+    dref = oracle.mesh_ft_backward_grid(w.vertices, w.faces, w.n, w.spacing, w.mode, Gs.astype(np.complex128), flat_indices=bidx)
+    gerr = _rel_l2(dv, dref)
+    report(f"cfg3 backward, cotangent on the complete x-rows {brows} ({len(bidx)} frequencies): rel L2 = {gerr:.2e}")
+    assert gerr <= GRAD_TOL, gerr
     plan.close()
 
 

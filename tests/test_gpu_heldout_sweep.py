@@ -130,12 +130,11 @@ def test_heldout_random_cases(seed):
         plan.close()
 
 
-def test_heldout_summary():
-    """Prints the worst case of every category (run with -s to see it; always recorded in the JUnit properties)."""
+def test_heldout_summary(report):
+    """Reports the worst case of every category (printed in the terminal summary through the ``report`` fixture)."""
     assert WORST, "the sweep did not run"
-    print()
     for cat in sorted(WORST):
         fe, ge, tf, tg = WORST[cat]
-        print(f"held-out sweep [{cat}]: worst forward {fe:.2e} (seed, case = {tf[:2] if tf else None}), "
+        report(f"held-out sweep [{cat}]: worst forward {fe:.2e} (seed, case = {tf[:2] if tf else None}), "
               f"worst gradient rel L2 {ge:.2e} (seed, case = {tg[:2] if tg else None})")
     assert all(w[0] <= FWD_TOL and w[1] <= GRAD_TOL for w in WORST.values())

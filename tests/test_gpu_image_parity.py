@@ -41,7 +41,7 @@ def _setup(dm, cfg):
     return w, plan, torch.as_tensor(w.vertices, device="cuda")
 
 
-def test_cfg2_render_l2_loss_and_backward_against_full_oracle(dm):
+def test_cfg2_render_l2_loss_and_backward_against_full_oracle(dm, report):
     import torch
     w, plan, vd = _setup(dm, 2)
     wt = build_workload(2, seed_offset=100)                      # the "second perturbed mesh" of the config (seed 101)
@@ -62,7 +62,7 @@ def test_cfg2_render_l2_loss_and_backward_against_full_oracle(dm):
     e_m = np.abs(m.cpu().numpy() - m_o).max() / np.abs(m_o).max()
     e_l = abs(loss - loss_o) / loss_o
     e_g = np.linalg.norm(dv - dv_o) / np.linalg.norm(dv_o)
-    print(f"cfg2: image max err {e_u:.2e} / {e_m:.2e} of the image max, loss rel err {e_l:.2e}, gradient rel L2 {e_g:.2e}")
+    report(f"cfg2: image max err {e_u:.2e} / {e_m:.2e} of the image max, loss rel err {e_l:.2e}, gradient rel L2 {e_g:.2e}")
     assert e_u <= IMG_TOL and e_m <= IMG_TOL
     assert e_l <= 1e-3
     assert e_g <= GRAD_TOL
@@ -70,7 +70,7 @@ def test_cfg2_render_l2_loss_and_backward_against_full_oracle(dm):
 
 
 @pytest.mark.parametrize("cfg", [3, 4, 5])
-def test_image_stages_against_numpy_fft_of_the_gpu_spectrum(dm, cfg):
+def test_image_stages_against_numpy_fft_of_the_gpu_spectrum(dm, cfg, report):
     import torch
     w, plan, vd = _setup(dm, cfg)
     cov = w.psf_cov
@@ -85,7 +85,7 @@ def test_image_stages_against_numpy_fft_of_the_gpu_spectrum(dm, cfg):
     G = plan.image_to_spectrum_cotangent(torch.as_tensor(g, device="cuda"), cov).cpu().numpy()
     Gref = oracle.image_to_spectrum_cotangent(g, w.n, w.spacing, w.origin, cov.astype(np.float64))
     e_cot = np.abs(G - Gref).max() / np.abs(Gref).max()
-    print(f"cfg{cfg}: image stage vs numpy irfftn of the GPU spectrum {e_img:.2e} of the image max; "
+    report(f"cfg{cfg}: image stage vs numpy irfftn of the GPU spectrum {e_img:.2e} of the image max; "
           f"adjoint stage vs numpy rfftn {e_cot:.2e} of max|G|")
     assert e_img <= STAGE_TOL
     assert e_cot <= STAGE_TOL
@@ -93,7 +93,7 @@ def test_image_stages_against_numpy_fft_of_the_gpu_spectrum(dm, cfg):
 
 
 @pytest.mark.parametrize("cfg", [3, 4])
-def test_render_fast_kernels_against_robust_kernels(dm, cfg):
+def test_render_fast_kernels_against_robust_kernels(dm, cfg, report):
     w, plan, vd = _setup(dm, cfg)
     img = plan.render(vd, w.psf_cov).clone()
     assert plan.paths_used()[0] == 0
@@ -101,6 +101,6 @@ def test_render_fast_kernels_against_robust_kernels(dm, cfg):
     ref = plan.render(vd, w.psf_cov)
     assert plan.paths_used()[0] == 1
     err = float((img - ref).abs().max() / ref.abs().max())
-    print(f"cfg{cfg}: whole render, fast vs robust kernels: {err:.2e} of the image max")
+    report(f"cfg{cfg}: whole render, fast vs robust kernels: {err:.2e} of the image max")
     assert err <= 0.5 * IMG_TOL
     plan.close()

@@ -392,6 +392,18 @@ def test_per_face_density_weights(dm, mode):
         assert np.abs(F - ref).max() <= FWD_TOL * abs(ref[0]), path
         dv = plan.mesh_ft_backward(_dev(v), _dev(G)).cpu().numpy()
         assert _rel_l2(dv, dref) <= GRAD_TOL, path
+    # the no-synchronisation update with a caller-asserted class: same routing and same bits as the classifying call
+    plan.set_option(dm.DM_OPT_FORWARD_PATH, 0)
+    plan.set_option(dm.DM_OPT_BACKWARD_PATH, 0)
+    for wset, robust in ((wts, True), (np.abs(wts) * 1.5, False)):        # mixed signs -> robust; one sign per component -> fast
+        plan.set_face_weights(_dev(wset))
+        Fa = plan.mesh_ft_forward(_dev(v))
+        dva = plan.mesh_ft_backward(_dev(v), _dev(G))
+        assert plan.paths_used() == ((1, 1) if robust else (0, 0))
+        plan.update_face_weights(_dev(np.ones_like(wset)), robust=False)    # something else in between
+        plan.update_face_weights(_dev(wset), robust=robust)
+        assert torch.equal(plan.mesh_ft_forward(_dev(v)), Fa) and torch.equal(plan.mesh_ft_backward(_dev(v), _dev(G)), dva)
+        assert plan.paths_used() == ((1, 1) if robust else (0, 0))
     plan.set_face_weights(None)
     F1 = plan.mesh_ft_forward(_dev(v)).cpu().numpy().reshape(-1)
     assert np.abs(F1 - oracle.mesh_ft_forward(v, f, k, mode)).max() <= FWD_TOL * abs(ref[0])

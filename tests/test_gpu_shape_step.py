@@ -65,8 +65,11 @@ def test_preconditioner_against_dense_solves(dm, cfg, sub):
     plan.close()
 
 
+@pytest.mark.parametrize("banded", [False, True])
 @pytest.mark.parametrize("mode", [0, 1])
-def test_three_shape_steps_against_the_oracle(dm, mode):
+def test_three_shape_steps_against_the_oracle(dm, mode, banded):
+    """``banded``: the step on the narrow band, against the oracle's band branch (pinned by finite
+    differences of the banded render in tests/test_oracle_shape.py)."""
     import torch
     w = build_workload(1, grid_override=(24, 24, 24))                 # 162 vertices, 320 triangles
     wt = build_workload(2, subdiv_override=2, grid_override=(24, 24, 24))   # target: a perturbed sphere of radius 0.35
@@ -74,6 +77,15 @@ def test_three_shape_steps_against_the_oracle(dm, mode):
     cov = np.array([cov[0], cov[1], cov[2], 0.0, 0.0, 0.0])
     target = oracle.render(wt.vertices, wt.faces, w.n, w.spacing, w.origin, cov, mode)
     plan = dm.Plan(w.n, w.spacing, w.origin, mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
+    band = None
+    if banded:
+        cutoff = 0.05
+        k = oracle.frequency_grid(w.n, w.spacing)
+        h = np.exp(-0.5 * (cov[0] * k[..., 0] ** 2 + cov[1] * k[..., 1] ** 2 + cov[2] * k[..., 2] ** 2))
+        assert np.abs(h / cutoff - 1.0).min() > 1e-3        # no frequency sits on the edge of the band: fp32 and fp64 agree on it
+        band = h > cutoff
+        assert 0.02 < band.mean() < 0.5
+        plan.set_narrow_band(cov, cutoff)
     lr = 2e-3
     st = plan.shape_state(lr=lr)
     ost = oracle.ShapeState()
@@ -85,12 +97,12 @@ def test_three_shape_steps_against_the_oracle(dm, mode):
         v_before = vd.cpu().numpy().astype(np.float64)
         loss = st.step(vd, td, cov, return_loss=True)
         v_new_o, loss_o = oracle.shape_step(v_o.astype(np.float32), w.faces, w.n, w.spacing, w.origin, cov, mode,
-                                            target.astype(np.float32), ost, prm)
+                                            target.astype(np.float32), ost, prm, band=band)
         v_gpu = vd.cpu().numpy().astype(np.float64)
         e_v = _rel(v_gpu, v_new_o)
         e_d = _rel(v_gpu - v_before, v_new_o - v_o.astype(np.float32).astype(np.float64))
         e_l = abs(loss - loss_o) / abs(loss_o)
-        print(f"mode {mode} step {step}: vertices rel {e_v:.2e}, displacement rel {e_d:.2e}, Phi_1 rel {e_l:.2e}")
+        print(f"mode {mode} banded {banded} step {step}: vertices rel {e_v:.2e}, displacement rel {e_d:.2e}, Phi_1 rel {e_l:.2e}")
         assert e_v <= 1e-4
         assert e_d <= 5e-3
         assert e_l <= 1e-3

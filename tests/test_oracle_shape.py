@@ -107,3 +107,73 @@ def test_shape_step_moves_towards_the_target_and_decreases_phi1():
     assert np.abs(np.linalg.norm(v1 - v, axis=1)).max() <= 5e-3 * np.sqrt(3) + 1e-12    # lr bounds every coordinate's move
     l1 = oracle.phi1(oracle.render(v1, f, n, spacing, origin, cov, 0), target)
     assert l1 < l0
+
+
+# ---- the step as a COMPOSITION (eq. 17; band: PAPER.md:227-240) -----------------------------------------
+# The pieces above are pinned one by one; what follows pins their order.  The gradient is re-derived here by central finite
+# differences of Phi_1 o render (forward evaluations only -- never oracle.render_backward), the preconditioner is the
+# tetrahedron's closed form, and AdamUniform's first step is lr * g~ / max|g~| (test_adam_uniform_steps_by_hand).  A step that
+# skipped the preconditioner, differentiated another loss, or banded F but not G would miss these by orders of magnitude.
+def _tetra_problem():
+    from workloads.configs import _grid
+    v, f = tetrahedron_mesh([[-0.2, -0.2, -0.2], [0.25, -0.15, -0.2], [-0.1, 0.3, -0.15], [0.0, 0.0, 0.3]])
+    n, spacing, origin = _grid((8, 8, 8))
+    cov = np.array([(1.2 * spacing[0]) ** 2, (1.0 * spacing[1]) ** 2, (1.5 * spacing[2]) ** 2, 0, 0, 0], dtype=np.float64)
+    target = oracle.render(1.2 * v + 0.01, f, n, spacing, origin, cov, 0)
+    return v, f, n, spacing, origin, cov, target
+
+
+def _band_mask(n, spacing, cov, cutoff):
+    k = oracle.frequency_grid(n, spacing)                               # [n_x, n_y, n_z/2+1, 3]
+    quad = cov[0] * k[..., 0] ** 2 + cov[1] * k[..., 1] ** 2 + cov[2] * k[..., 2] ** 2
+    return np.exp(-0.5 * quad) > cutoff
+
+
+def _fd_gradient(loss_of_vertices, v, h=1e-6):
+    g = np.zeros_like(v)
+    for i in range(v.shape[0]):
+        for d in range(3):
+            vp, vm = v.copy(), v.copy()
+            vp[i, d] += h
+            vm[i, d] -= h
+            g[i, d] = (loss_of_vertices(vp) - loss_of_vertices(vm)) / (2 * h)
+    return g
+
+
+@pytest.mark.parametrize("lam", [0.0, 50.0])
+def test_first_shape_step_equals_the_preconditioned_finite_difference_gradient(lam):
+    v, f, n, spacing, origin, cov, target = _tetra_problem()
+    g = _fd_gradient(lambda x: oracle.phi1(oracle.render(x, f, n, spacing, origin, cov, 0), target), v)
+    gp = g.mean(axis=0) + (g - g.mean(axis=0)) / (1 + 4 * lam) ** 2     # (I + lam L)^-2 on the tetrahedron, L = 4I - J
+    lr = 2e-3
+    want = v - lr * gp / np.abs(gp).max()
+    v1, loss = oracle.shape_step(v, f, n, spacing, origin, cov, 0, target, oracle.ShapeState(),
+                                 oracle.ShapeParams(lr=lr, lam=lam, eps=0.0))
+    assert loss == oracle.phi1(oracle.render(v, f, n, spacing, origin, cov, 0), target)
+    assert np.abs(v1 - want).max() <= 1e-5 * lr, np.abs(v1 - want).max() / lr
+    if lam > 0:   # the preconditioner matters: the unpreconditioned step is somewhere else entirely
+        assert np.abs(want - (v - lr * g / np.abs(g).max())).max() > 1e-2 * lr
+
+
+def test_shape_step_band_branch():
+    v, f, n, spacing, origin, cov, target = _tetra_problem()
+    prm = oracle.ShapeParams(lr=2e-3, lam=50.0, eps=0.0)
+    plain, loss_plain = oracle.shape_step(v, f, n, spacing, origin, cov, 0, target, oracle.ShapeState(), prm)
+    full = np.ones((n[0], n[1], n[2] // 2 + 1), dtype=bool)
+    allin, loss_all = oracle.shape_step(v, f, n, spacing, origin, cov, 0, target, oracle.ShapeState(), prm, band=full)
+    assert np.array_equal(plain, allin) and loss_plain == loss_all      # an all-true band is no band, bit for bit
+    band = _band_mask(n, spacing, cov, 0.05)
+    assert 0.04 < band.mean() < 0.6 and band[0, 0, 0]                   # a real restriction that keeps k = 0
+
+    def banded_loss(x):
+        F = oracle.mesh_ft_forward_grid(x, f, n, spacing, 0)
+        return oracle.phi1(oracle.spectrum_to_image(np.where(band, F, 0.0), n, spacing, origin, cov), target)
+
+    g = _fd_gradient(banded_loss, v)
+    gp = g.mean(axis=0) + (g - g.mean(axis=0)) / (1 + 4 * prm.lam) ** 2
+    want = v - prm.lr * gp / np.abs(gp).max()
+    got, loss = oracle.shape_step(v, f, n, spacing, origin, cov, 0, target, oracle.ShapeState(), prm, band=band)
+    assert loss == banded_loss(v)
+    assert np.abs(got - want).max() <= 1e-5 * prm.lr, np.abs(got - want).max() / prm.lr
+    # and the band is not a no-op here: the unbanded step differs visibly
+    assert np.abs(got - plain).max() > 1e-3 * prm.lr
