@@ -37,6 +37,18 @@ FLOOR_OPS = {"fwd": {0: 26.0, 1: 23.0}, "bwd": {0: 60.0, 1: 60.0}}
 FP32_LANES_PER_CLK_PER_SM = 128
 
 
+def _cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    import platform
+    return platform.processor() or platform.machine() or "unknown"
+
+
 def _peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -187,7 +199,7 @@ def run_reference(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "cfg": args.cfg, "mode": "surface" if w.mode else "volume",
                    "n_triangles": int(w.faces.shape[0]), "grid": list(w.n), "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": res[0]["cores"], "kind": "oracle", "sample": sample,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": res[0]["cores"], "cpu_model": _cpu_model(), "kind": "oracle", "sample": sample,
                          "fwd_pairs_s": res[0]["pairs"] / np.mean([r["fwd_s"] for r in res]),
                          "bwd_pairs_s": res[0]["pairs"] / np.mean([r["bwd_s"] for r in res])},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -216,9 +228,9 @@ def run_sharded(args):
     torch.cuda.set_device(local)
     dm.load_library()
     if world > 1:
-        os.environ.setdefault("NCCL_DEBUG", "INFO")   # which algorithm / transport (NVLS, P2P) the collectives took
-        os.environ.setdefault("NCCL_DEBUG_FILE", os.path.join(ROOT, "gpurun_out", "nccl_rank%h_%p.log"))
-        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        # which algorithm / transport (NVLS, P2P) the collectives took; left on stderr so that whoever launched the ranks
+        # sees the communicator lines of every rank
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     w = build_workload(args.cfg)                      # the same mesh on every rank
     plan = dm.Plan(w.n, w.spacing, w.origin, w.mode, torch.as_tensor(w.faces, device="cuda"), w.vertices.shape[0])
@@ -283,10 +295,23 @@ def run_sharded(args):
         e2e_step()
     e1.record(stream)
     barrier()
-    t = torch.tensor([fwd_ms + bwd_ms, fwd_ms, bwd_ms, e0.elapsed_time(e1) / e2e_n], dtype=torch.float64, device="cuda")
+    # the other way to use N GPUs, for comparison: every rank the WHOLE problem on its own (no collective), weak scaling
+    r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    plan.mesh_ft_forward(vd, out=F)
+    plan.mesh_ft_backward(vd, Gd)
+    barrier()
+    r0.record(stream)
+    for _ in range(e2e_n):
+        flush.fill_(1)
+        plan.mesh_ft_forward(vd, out=F)
+        plan.mesh_ft_backward(vd, Gd)
+    r1.record(stream)
+    barrier()
+    t = torch.tensor([fwd_ms + bwd_ms, fwd_ms, bwd_ms, e0.elapsed_time(e1) / e2e_n, r0.elapsed_time(r1) / e2e_n],
+                     dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    step_ms, fwd_ms, bwd_ms, e2e_ms = (float(x) for x in t.tolist())
+    step_ms, fwd_ms, bwd_ms, e2e_ms, rep_ms = (float(x) for x in t.tolist())
     if rank == 0:
         sm_max_mhz, peak_src = _peaks()
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
@@ -307,6 +332,8 @@ def run_sharded(args):
                     "what": "sharded forward + all-gather + image stage, cotangent stage + sharded backward + all-reduce, "
                             "pinned host buffers in and out on every rank"},
             "gpu_launches": int(launches), "clocks": clk.summary(),
+            "replicas": {"value": world * pairs / (rep_ms * 1e-3), "unit": UNIT, "ms_per_step": rep_ms, "scaling": "weak",
+                         "steps": e2e_n, "what": "every rank the whole problem on its own, no collective (includes the L2 flush)"},
             "roofline": {"bound": "alu", "kernel": "dm_k_backward_fast + all-reduce (whole sharded backward)",
                          "achieved": achieved, "peak": peak, "unit": "T lane-op/s over all ranks", "frac": achieved / peak,
                          "traffic": None, "peak_source": f"{world} x 128 x {n_sm} SMs x {sm_max_mhz:.0f} MHz ({peak_src})"},
@@ -465,10 +492,16 @@ def run_ours(args):
             "peak_source": f"128 x {n_sm} SMs x {sm_max_mhz:.0f} MHz ({peak_src}); DESIGN.md section 7",
             "frac_at_measured_clock": achieved / (peak * sm_mhz / sm_max_mhz),
             "algorithmic_ops_per_pair": FLOOR_OPS["bwd"][w.mode], "kernel_ms": bk_ms,
-            "forward": {"achieved": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12,
-                        "frac": FLOOR_OPS["fwd"][w.mode] * pairs / (fwd_ms * 1e-3) / 1e12 / peak,
-                        "algorithmic_ops_per_pair": FLOOR_OPS["fwd"][w.mode]},
         }
+        # forward: the strip walk issues fewer instructions per pair than the itemised per-pair floor (it shares vertex work
+        # along the strip), so the fraction is taken against min(floor, issued): it can never exceed the issue utilisation
+        fwd_issued = ((ncu or {}).get("forward") or {}).get("issued_instr_per_pair_full_grid") if w.cfg == 4 else None
+        fwd_ops = min(FLOOR_OPS["fwd"][w.mode], fwd_issued) if fwd_issued else FLOOR_OPS["fwd"][w.mode]
+        roofline["forward"] = {"achieved": fwd_ops * pairs / (fwd_ms * 1e-3) / 1e12,
+                               "frac": fwd_ops * pairs / (fwd_ms * 1e-3) / 1e12 / peak,
+                               "algorithmic_ops_per_pair": fwd_ops, "itemised_floor_ops_per_pair": FLOOR_OPS["fwd"][w.mode],
+                               "issued_instr_per_pair": fwd_issued,
+                               "note": "ops per pair = min(itemised floor, issued instructions per pair measured by ncu at cfg 4)"}
         if ncu:
             roofline["ncu"] = ncu
         # the other full-size configs (volume mode carries 5 more operations per pair against the same floor)
@@ -502,13 +535,15 @@ def run_ours(args):
                        "parallelism": f"replicas x{world}"},
             "fwd_pairs_s": world * pairs / (fwd_ms * 1e-3), "bwd_pairs_s": world * pairs / (bwd_ms * 1e-3),
             "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
+            "fwd_ms_median": float(np.median([e[0].elapsed_time(e[1]) for e in evs])),
+            "bwd_ms_median": float(np.median([e[1].elapsed_time(e[2]) for e in evs])),
             "render_ms": float(np.median(render_ms)), "render_stage_ms": stage,
             "e2e": {"value": world * pairs / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
                     "what": "dm_render + dm_render_backward with pinned host vertices/dL_dimage in, image/dL_dv out"},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
             "cpu_baseline": {"value": o["pairs"] / (o["fwd_s"] + o["bwd_s"]), "unit": UNIT, "cores": o["cores"],
-                             "kind": "oracle", "sample": sample, "fwd_pairs_s": o["pairs"] / o["fwd_s"],
+                             "cpu_model": _cpu_model(), "kind": "oracle", "sample": sample, "fwd_pairs_s": o["pairs"] / o["fwd_s"],
                              "bwd_pairs_s": o["pairs"] / o["bwd_s"],
                              "single_thread": None if o1 is None else {
                                  "value": o1["pairs"] / (o1["fwd_s"] + o1["bwd_s"]), "cores": o1["cores"],
@@ -532,14 +567,21 @@ def main():
     ap.add_argument("--cfg", type=int, default=4, help="BASELINE.json config 1..5 (default 4, the target config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-freqs", type=int, default=192, help="stored frequencies per oracle sample")
-    ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"],
-                    help="replicas (default): every rank its own problem, weak scaling, no data-path collective; slab: ONE problem "
-                         "sharded by x-slab of the stored spectrum (all-gather of F, all-reduce of dL/dv), strong scaling")
+    ap.add_argument("--shard", default="auto", choices=["auto", "replicas", "slab"],
+                    help="slab: ONE problem sharded by x-slab of the stored spectrum (all-gather of F, all-reduce of dL/dv over "
+                         "NCCL), strong scaling, with the replica figure under the key 'replicas'; replicas: every rank its own "
+                         "problem, weak scaling, no data-path collective; auto (default): replicas at --gpus 1, slab above")
     ap.add_argument("--extra-cfgs", default="1,2,3,5", help="other BASELINE.json configs timed (N=1 only) for the extra roofline "
                     "entries; '' switches them off")
     ap.add_argument("--x-slab", default="", help="a:b -- profiling aid (ncu counters overflow on the 0.4 s full-grid launch): run "
                     "forward/backward on rows [a,b) of the spectrum only and print a short line that is NOT a bench result")
     args = ap.parse_args()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.shard == "auto":
+        args.shard = "slab" if max(args.gpus, world) > 1 else "replicas"
+    if args.impl == "ours" and args.gpus != world:
+        raise SystemExit(f"bench.py --gpus {args.gpus} must be launched with one process per GPU (python -m torch.distributed.run "
+                         f"--nproc-per-node {args.gpus} ... bench.py --gpus {args.gpus}); this process sees WORLD_SIZE={world}")
     if args.impl == "reference":
         run_reference(args)
     elif args.shard == "slab":

@@ -28,3 +28,23 @@ def test_non_zero_ranks_of_the_reference_arm_exit_quietly():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"], capture_output=True,
                          text=True, timeout=120, cwd=ROOT, env=env)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_our_arm_fails_loudly_without_cuda_or_without_its_ranks():
+    """No CUDA device here: the product arm must refuse (no CPU fallback, no JSON line) -- at one rank, and as rank 0 of a
+    two-rank launch (the x-slab leg); --gpus 2 outside torchrun is refused before anything runs."""
+    import torch
+    if torch.cuda.is_available():
+        import pytest
+        pytest.skip("a CUDA device is present")
+    bench = os.path.join(ROOT, "bench.py")
+    base = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    for extra_env, argv in (({}, ["--steps", "1", "--warmup", "0"]),
+                            ({"RANK": "0", "WORLD_SIZE": "2", "LOCAL_RANK": "0", "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": "29999"},
+                             ["--gpus", "2", "--steps", "1", "--warmup", "0"]),
+                            ({}, ["--gpus", "2"])):
+        out = subprocess.run([sys.executable, bench] + argv, capture_output=True, text=True, timeout=300, cwd=ROOT,
+                             env=dict(base, **extra_env))
+        assert out.returncode != 0, (argv, out.stdout)
+        assert not [ln for ln in out.stdout.splitlines() if ln.startswith("{")], out.stdout
+        assert "CUDA" in out.stderr or "one process per GPU" in out.stderr, out.stderr[-400:]
