@@ -9,7 +9,8 @@ Parity status: every function here is pinned by `-m "not gpu"` tests (tests/test
 the behaviour of an inverse real FFT on a half spectrum that is not exactly Hermitian on its
 self-conjugate planes (reading R13), where the oracle *defines* the semantics as numpy/pocketfft's
 irfftn -- "parity unpinned" for that one convention.  oracle/shape_step.py (the shape-optimisation step of PAPER.md:244-249) is
-pinned by tests/test_oracle_shape.py.
+pinned by tests/test_oracle_shape.py, piece by piece and as a composition (the first step against finite differences of
+Phi_1 o render with the closed-form preconditioner of the tetrahedron, and its band branch against the banded render).
 """
 from .mesh_ft import (  # noqa: F401
     frequency_grid,
